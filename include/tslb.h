@@ -1,0 +1,125 @@
+/*
+ * tslb.h -- C ABI of the B200-native thread-safe lattice Boltzmann (TSLB) two-component time
+ * step of arxiv 2403.15773 ("PAPER.md" below = /root/reference/PAPER.md; readings A1..A17 are
+ * listed in DESIGN.md §3).
+ *
+ * One context owns the state of one simulation on one CUDA device:
+ *   per lattice node   rho, u = (ux,uy,uz), Pi^neq = (xx,yy,zz,xy,xz,yz)   [PAPER.md:108]
+ *   and, if two_component, the phase field phi                              [PAPER.md:198-211]
+ * double-buffered in device memory (HBM).  No populations f_i are ever stored.  tslb_step()
+ * advances all nodes by n time steps; per step every node pulls its 26 neighbours' stored moments,
+ * rebuilds their post-collision D3Q27 populations f^eq + (1-omega) f^neq with the third-order
+ * Hermite expansion (eq. 5, 98 eq. 6, 166 eq. 16, 183 eq. 19), takes the moments of
+ * the streamed populations, and advances phi by the D3Q7 LB of PAPER.md:206-211
+ * eqs. 23-24 with the surface-tension force F = sigma kappa grad(phi) (PAPER.md:192-196
+ * eqs. 20-21) applied as a velocity kick.  Every step runs in hand-written CUDA kernels for
+ * sm_100a; there is no CPU fallback.
+ *
+ * Conventions
+ *   - Every function returns TSLB_OK (0) or a negative error code; nothing throws or aborts.
+ *     tslb_last_error() returns a human-readable description of the last failure.
+ *   - Field arrays passed in/out are DENSE, x fastest: element (x,y,z) at x + nx*(y + ny*z),
+ *     nx*ny*nz elements of the context's precision (float for TSLB_F32, double for TSLB_F64).
+ *   - Pointers are HOST pointers when pointers_on_device == 0 and DEVICE pointers (same device
+ *     as the context) when it is 1.  The caller owns every buffer it passes; the library copies
+ *     in / out and keeps no caller pointer except `workspace` and `stream`.
+ *   - All device work is enqueued on `stream`.  tslb_step() is asynchronous; tslb_get_moments()
+ *     synchronises the stream before returning.
+ *   - x and y are always periodic.  z is periodic, or jet inflow at z = 0 with outflow at
+ *     z = nz-1 (eqs. 9-10, 223).
+ */
+#ifndef TSLB_H
+#define TSLB_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tslb_ctx tslb_ctx; /* opaque, owned by the library */
+
+enum { TSLB_OK = 0, TSLB_EINVAL = -1, TSLB_ENOMEM = -2, TSLB_ECUDA = -3, TSLB_ESTATE = -4 };
+enum { TSLB_F32 = 0, TSLB_F64 = 1 };
+enum { TSLB_BC_PERIODIC = 0, TSLB_BC_JET_INFLOW = 1, TSLB_BC_OUTFLOW = 2 };
+/* kernel selection (tslb_params.kernel) */
+enum {
+  TSLB_KERNEL_AUTO = 0,     /* fastest kernel that supports the grid                           */
+  TSLB_KERNEL_GENERIC = 1,  /* one thread per node, direct global loads; any grid size         */
+  TSLB_KERNEL_TILED = 2     /* TMA-staged x-y tiles marching along z; needs nx, ny multiples of
+                               the tile (tslb_create fails with TSLB_EINVAL otherwise)          */
+};
+
+typedef struct {
+  int nx, ny, nz;          /* grid.  All > 0; nz >= 4 if z is not periodic */
+  int precision;           /* TSLB_F32 | TSLB_F64: element type of every field pointer and
+                              the arithmetic type of the kernels                               */
+  int two_component;       /* 0: flow only; 1: flow + phase field           */
+  int hermite_order;       /* 3: eqs. 16 and 19 (the paper's scheme); 2: eq. 8                 */
+  double omega;            /* relaxation frequency, 0 < omega < 2;
+                              nu = c_s^2 (1/omega - 1/2), c_s^2 = 1/3            */
+  double sigma;            /* surface tension of eq. 20                         */
+  double interface_width;  /* W > 0: equilibrium profile phi = 1/2 (1 + tanh(2 s / W));
+                              anti-diffusion gamma of eq. 24 is 2/W (reading A8)               */
+  int bc_zlo, bc_zhi;      /* TSLB_BC_PERIODIC / TSLB_BC_PERIODIC, or
+                              TSLB_BC_JET_INFLOW / TSLB_BC_OUTFLOW                             */
+  double jet_diameter;     /* D: nozzle disc (x-(nx-1)/2)^2 + (y-(ny-1)/2)^2 < (D/2)^2 on z=0  */
+  double jet_velocity;     /* U: inflow u_z = U (1 + jet_perturbation * xi)                    */
+  double jet_perturbation; /* amplitude of the seeded uniform perturbation xi in (-1,1) (A12)  */
+  unsigned long long seed; /* seed of the counter-based inflow hash                            */
+  int device;              /* CUDA device ordinal                                              */
+  int kernel;              /* TSLB_KERNEL_*                                                    */
+  void *stream;            /* cudaStream_t of the caller (NULL = legacy default stream)        */
+  void *workspace;         /* optional caller-owned DEVICE memory, 256-byte aligned (e.g. a
+                              torch tensor); NULL -> the library allocates with cudaMalloc     */
+  size_t workspace_bytes;  /* size of `workspace`; must be >= tslb_workspace_bytes()           */
+} tslb_params;
+
+/* Device bytes the context needs: 2 x (10 moment arrays [+ phi]) in the padded internal layout
+ * (x/y ghost cells for the periodic wrap).  0 if the parameters are invalid.     */
+size_t tslb_workspace_bytes(const tslb_params *p);
+
+/* Validate parameters, select the device, allocate (or adopt) the workspace, build the TMA
+ * descriptors.  On failure *out is NULL and, if out_err is passed to tslb_last_error(NULL), the
+ * message of the failed create is returned.                                                     */
+int tslb_create(const tslb_params *p, tslb_ctx **out);
+
+/* Set the time-0 state and reset the step counter.  rho, ux, uy, uz: required.  phi: required
+ * iff two_component (else must be NULL).  pineq: NULL (-> Pi^neq = 0, a plain equilibrium start)
+ * or 6 pointers xx,yy,zz,xy,xz,yz.  With inflow/outflow the two z boundary planes are then set
+ * from the initial fields as in a step (hash step index 0).                                     */
+int tslb_init_fields(tslb_ctx *c, const void *rho, const void *ux, const void *uy, const void *uz,
+                     const void *phi, const void *const pineq[6], int pointers_on_device);
+
+/* Advance nsteps >= 0 time steps (eq. 6 + 206 eq. 23 per step).  Asynchronous on
+ * the context's stream.  TSLB_ESTATE before tslb_init_fields.                                   */
+int tslb_step(tslb_ctx *c, int nsteps);
+
+/* Copy out the stored state: rho, the stored (post-kick) velocity u' (the time-centred physical
+ * velocity is u' - F/(2 rho), reading A9), Pi^neq (NOT the full Pi; reading A2) and phi.  Any
+ * pointer (and any entry of pineq, or pineq itself) may be NULL.  Synchronises the stream.      */
+int tslb_get_moments(tslb_ctx *c, void *rho, void *ux, void *uy, void *uz, void *const pineq[6],
+                     void *phi, int pointers_on_device);
+
+/* Number of time steps taken since tslb_init_fields (keys the inflow hash).                     */
+long long tslb_step_count(const tslb_ctx *c);
+
+/* Name of the kernel tslb_step launches for this context ("generic", "tiled<64x8>", ...) and the
+ * number of kernel launches it has made so far (for benchmark bookkeeping).                     */
+const char *tslb_kernel_name(const tslb_ctx *c);
+long long tslb_launch_count(const tslb_ctx *c);
+
+/* Inflow perturbation xi(seed, x, y, step) in (-1,1) evaluated ON THE DEVICE for x in [0,nx),
+ * y in [0,ny) into out[nx*ny] doubles (host pointer) -- test probe for the bit-exact hash pin.  */
+int tslb_debug_xi(tslb_ctx *c, long long step, double *out_host);
+
+int tslb_destroy(tslb_ctx *c);
+
+/* Last error message of the context (or of the last failed tslb_create when c == NULL).
+ * The string is owned by the library and valid until the next call on the same context/thread.  */
+const char *tslb_last_error(const tslb_ctx *c);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TSLB_H */

@@ -1,0 +1,398 @@
+// tslb_api.cu -- the C-ABI boundary (include/tslb.h): context, validation, workspace carving,
+// field import/export, kernel dispatch.  Host-side bookkeeping only; every step of the method
+// runs in the kernels of tslb_generic.cuh / tslb_tiled.cuh.
+#include <cuda_runtime.h>
+
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "../../include/tslb.h"
+#include "tslb_generic.cuh"
+#include "tslb_tiled.cuh"
+
+using namespace tslb;
+
+namespace {
+
+thread_local std::string g_create_error;
+
+size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+Layout make_layout(int nx, int ny, int nz) {
+  Layout L;
+  L.nx = nx; L.ny = ny; L.nz = nz;
+  L.px = nx + 2 * GX;
+  L.py = ny + 2 * GY;
+  L.plane = (long long)L.px * L.py;
+  L.field = (long long)round_up((size_t)L.plane * nz, 64);
+  return L;
+}
+
+struct Validated {
+  bool ok = false;
+  std::string why;
+  bool zper = true;
+  int kernel = TSLB_KERNEL_GENERIC;   // resolved kernel
+  size_t esize = 4;
+  int nfields = 10;
+  Layout L{};
+  size_t bytes = 0;
+};
+
+Validated validate(const tslb_params *p) {
+  Validated v;
+  auto fail = [&](const char *m) { v.ok = false; v.why = m; return v; };
+  if (!p) return fail("params is NULL");
+  if (p->nx <= 0 || p->ny <= 0 || p->nz <= 0) return fail("grid sizes must be positive");
+  if ((long long)p->nx * p->ny * p->nz > (1LL << 40)) return fail("grid too large");
+  if (p->precision != TSLB_F32 && p->precision != TSLB_F64) return fail("precision must be TSLB_F32 or TSLB_F64");
+  if (p->hermite_order != 2 && p->hermite_order != 3) return fail("hermite_order must be 2 or 3");
+  if (!(p->omega > 0.0 && p->omega < 2.0)) return fail("omega must be in (0,2)");
+  if (p->two_component && !(p->interface_width > 0.0)) return fail("interface_width must be > 0 when two_component");
+  const bool zper = p->bc_zlo == TSLB_BC_PERIODIC && p->bc_zhi == TSLB_BC_PERIODIC;
+  const bool jet = p->bc_zlo == TSLB_BC_JET_INFLOW && p->bc_zhi == TSLB_BC_OUTFLOW;
+  if (!zper && !jet) return fail("boundary types must be PERIODIC/PERIODIC or JET_INFLOW/OUTFLOW");
+  if (jet && p->nz < 4) return fail("nz >= 4 is required with inflow/outflow");
+  if (jet && !(p->jet_diameter >= 0.0)) return fail("jet_diameter must be >= 0");
+  if (p->kernel < TSLB_KERNEL_AUTO || p->kernel > TSLB_KERNEL_TILED) return fail("unknown kernel selector");
+  v.zper = zper;
+  v.esize = p->precision == TSLB_F32 ? 4 : 8;
+  v.nfields = p->two_component ? 11 : 10;
+  v.L = make_layout(p->nx, p->ny, p->nz);
+  const bool tiled_ok = tiled_supported(p->precision, p->nx, p->ny, p->nz);
+  if (p->kernel == TSLB_KERNEL_TILED && !tiled_ok)
+    return fail("TSLB_KERNEL_TILED needs nx and ny to be multiples of the tile (see tslb_tiled.cuh)");
+  v.kernel = (p->kernel == TSLB_KERNEL_GENERIC || !tiled_ok) ? TSLB_KERNEL_GENERIC : TSLB_KERNEL_TILED;
+  // 2 buffers x nfields arrays, + 3 scratch arrays for the generic two-component path
+  size_t narr = 2 * (size_t)v.nfields;
+  if (v.kernel == TSLB_KERNEL_GENERIC && p->two_component) narr += 3;
+  v.bytes = narr * round_up((size_t)v.L.field * v.esize, 256);
+  v.ok = true;
+  return v;
+}
+
+}  // namespace
+
+struct tslb_ctx {
+  tslb_params p;
+  Validated v;
+  cudaStream_t stream = nullptr;
+  void *ws = nullptr;
+  bool own_ws = false;
+  void *fields[2][NF_MAX] = {};
+  void *nrm[3] = {};
+  int cur = 0;                 // index of the buffer holding time t
+  bool inited = false;
+  long long t = 0;
+  long long launches = 0;
+  void *stage = nullptr;       // one dense field, for host <-> device import/export
+  TiledPlan tiled;             // TMA descriptors etc.
+  std::string err;
+  std::string kname;
+
+  int fail(int code, const char *fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    err = buf;
+    return code;
+  }
+  int cuda_fail(cudaError_t e, const char *what) {
+    return fail(TSLB_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+  }
+};
+
+#define CK(call)                                             \
+  do {                                                       \
+    cudaError_t e_ = (call);                                 \
+    if (e_ != cudaSuccess) return c->cuda_fail(e_, #call);   \
+  } while (0)
+
+namespace {
+
+template <typename T>
+StepParams<T> make_step_params(tslb_ctx *c, int src, int dst) {
+  StepParams<T> P;
+  P.L = c->v.L;
+  for (int k = 0; k < NF_MAX; ++k) {
+    P.in.f[k] = (T *)c->fields[src][k];
+    P.out.f[k] = (T *)c->fields[dst][k];
+  }
+  for (int k = 0; k < 3; ++k) P.nrm[k] = (T *)c->nrm[k];
+  P.omc = (T)(1.0 - c->p.omega);
+  P.sigma = (T)(c->p.two_component ? c->p.sigma : 0.0);
+  P.gamma = (T)(c->p.two_component ? 2.0 / c->p.interface_width : 0.0);
+  P.zper = c->v.zper ? 1 : 0;
+  P.jetD2 = c->p.jet_diameter * c->p.jet_diameter;
+  P.jetU = (T)c->p.jet_velocity;
+  P.jetP = (T)c->p.jet_perturbation;
+  P.seed = c->p.seed;
+  P.step_next = c->t + 1;
+  return P;
+}
+
+template <typename T>
+int launch_generic(tslb_ctx *c, const StepParams<T> &P) {
+  const Layout &L = P.L;
+  const bool two = c->p.two_component != 0;
+  if (two) {
+    dim3 b(32, 8), g((L.nx + 31) / 32, (L.ny + 7) / 8, L.nz);
+    phase_normals_kernel<T><<<g, b, 0, c->stream>>>(P);
+    c->launches++;
+  }
+  dim3 b(32, 4), g((L.nx + 31) / 32, (L.ny + 3) / 4, L.nz);
+  const int o3 = c->p.hermite_order >= 3;
+  if (two) {
+    if (o3) generic_step_kernel<T, 3, true><<<g, b, 0, c->stream>>>(P);
+    else generic_step_kernel<T, 2, true><<<g, b, 0, c->stream>>>(P);
+  } else {
+    if (o3) generic_step_kernel<T, 3, false><<<g, b, 0, c->stream>>>(P);
+    else generic_step_kernel<T, 2, false><<<g, b, 0, c->stream>>>(P);
+  }
+  c->launches++;
+  CK(cudaGetLastError());
+  return TSLB_OK;
+}
+
+template <typename T>
+int step_typed(tslb_ctx *c, int nsteps) {
+  for (int s = 0; s < nsteps; ++s) {
+    StepParams<T> P = make_step_params<T>(c, c->cur, c->cur ^ 1);
+    int rc;
+    if (c->v.kernel == TSLB_KERNEL_TILED) {
+      cudaError_t e = launch_tiled<T>(c->tiled, P, c->cur, c->p.hermite_order, c->p.two_component != 0, c->stream);
+      c->launches++;
+      rc = (e == cudaSuccess) ? TSLB_OK : c->cuda_fail(e, "launch_tiled");
+    } else {
+      rc = launch_generic<T>(c, P);
+    }
+    if (rc != TSLB_OK) return rc;
+    c->cur ^= 1;
+    c->t++;
+  }
+  return TSLB_OK;
+}
+
+template <typename T>
+int fill_all_ghosts(tslb_ctx *c, int buf) {
+  const Layout &L = c->v.L;
+  dim3 b(128), g((L.px + 127) / 128, L.py, L.nz);
+  for (int k = 0; k < c->v.nfields; ++k) fill_ghosts_kernel<T><<<g, b, 0, c->stream>>>(L, (T *)c->fields[buf][k]);
+  CK(cudaGetLastError());
+  return TSLB_OK;
+}
+
+template <typename T>
+int init_typed(tslb_ctx *c, const void *const src[NF_MAX], int on_device) {
+  const Layout &L = c->v.L;
+  const size_t N = (size_t)L.nx * L.ny * L.nz;
+  dim3 b(128), g((L.nx + 127) / 128, L.ny, L.nz);
+  for (int k = 0; k < c->v.nfields; ++k) {
+    const T *d = nullptr;
+    if (src[k]) {
+      if (on_device) {
+        d = (const T *)src[k];
+      } else {
+        CK(cudaMemcpyAsync(c->stage, src[k], N * sizeof(T), cudaMemcpyHostToDevice, c->stream));
+        d = (const T *)c->stage;
+      }
+    }
+    pack_in_kernel<T><<<g, b, 0, c->stream>>>(L, d, (T *)c->fields[0][k], k == F_DRHO, d == nullptr);
+    CK(cudaGetLastError());
+    if (!on_device && src[k]) CK(cudaStreamSynchronize(c->stream));   // stage is reused
+  }
+  c->cur = 0;
+  c->t = 0;
+  if (!c->v.zper) {
+    StepParams<T> P = make_step_params<T>(c, 0, 0);
+    dim3 gb((L.nx + 127) / 128, L.ny, 2);
+    boundary_init_kernel<T><<<gb, b, 0, c->stream>>>(P, c->p.two_component);
+    CK(cudaGetLastError());
+  }
+  int rc = fill_all_ghosts<T>(c, 0);
+  if (rc != TSLB_OK) return rc;
+  // the other buffer's ghosts/halo start from a defined state too
+  for (int k = 0; k < c->v.nfields; ++k)
+    CK(cudaMemsetAsync(c->fields[1][k], 0, (size_t)L.field * sizeof(T), c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  return TSLB_OK;
+}
+
+template <typename T>
+int get_typed(tslb_ctx *c, void *const dst[NF_MAX], int on_device) {
+  const Layout &L = c->v.L;
+  const size_t N = (size_t)L.nx * L.ny * L.nz;
+  dim3 b(128), g((L.nx + 127) / 128, L.ny, L.nz);
+  for (int k = 0; k < c->v.nfields; ++k) {
+    if (!dst[k]) continue;
+    T *d = on_device ? (T *)dst[k] : (T *)c->stage;
+    pack_out_kernel<T><<<g, b, 0, c->stream>>>(L, (const T *)c->fields[c->cur][k], d, k == F_DRHO);
+    CK(cudaGetLastError());
+    if (!on_device) {
+      CK(cudaMemcpyAsync(dst[k], c->stage, N * sizeof(T), cudaMemcpyDeviceToHost, c->stream));
+      CK(cudaStreamSynchronize(c->stream));
+    }
+  }
+  CK(cudaStreamSynchronize(c->stream));
+  return TSLB_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t tslb_workspace_bytes(const tslb_params *p) {
+  Validated v = validate(p);
+  return v.ok ? v.bytes : 0;
+}
+
+int tslb_create(const tslb_params *p, tslb_ctx **out) {
+  if (!out) { g_create_error = "out is NULL"; return TSLB_EINVAL; }
+  *out = nullptr;
+  Validated v = validate(p);
+  if (!v.ok) { g_create_error = v.why; return TSLB_EINVAL; }
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev == 0) {
+    g_create_error = std::string("no CUDA device available (there is no CPU fallback): ") + cudaGetErrorString(e);
+    return TSLB_ECUDA;
+  }
+  if (p->device < 0 || p->device >= ndev) { g_create_error = "device ordinal out of range"; return TSLB_EINVAL; }
+  e = cudaSetDevice(p->device);
+  if (e != cudaSuccess) { g_create_error = std::string("cudaSetDevice: ") + cudaGetErrorString(e); return TSLB_ECUDA; }
+  cudaDeviceProp prop;
+  cudaGetDeviceProperties(&prop, p->device);
+  if (prop.major != 10) {
+    g_create_error = "this library is built for sm_100a (B200) only";
+    return TSLB_ECUDA;
+  }
+  tslb_ctx *c = new (std::nothrow) tslb_ctx();
+  if (!c) { g_create_error = "out of host memory"; return TSLB_ENOMEM; }
+  c->p = *p;
+  c->v = v;
+  c->stream = (cudaStream_t)p->stream;
+  if (p->workspace) {
+    if (p->workspace_bytes < v.bytes || ((uintptr_t)p->workspace & 255)) {
+      g_create_error = "workspace too small or not 256-byte aligned";
+      delete c;
+      return TSLB_EINVAL;
+    }
+    c->ws = p->workspace;
+  } else {
+    e = cudaMalloc(&c->ws, v.bytes);
+    if (e != cudaSuccess) {
+      g_create_error = std::string("cudaMalloc(workspace): ") + cudaGetErrorString(e);
+      delete c;
+      return TSLB_ENOMEM;
+    }
+    c->own_ws = true;
+  }
+  const size_t fb = round_up((size_t)v.L.field * v.esize, 256);
+  char *base = (char *)c->ws;
+  size_t off = 0;
+  for (int b = 0; b < 2; ++b)
+    for (int k = 0; k < v.nfields; ++k) { c->fields[b][k] = base + off; off += fb; }
+  if (v.kernel == TSLB_KERNEL_GENERIC && p->two_component)
+    for (int k = 0; k < 3; ++k) { c->nrm[k] = base + off; off += fb; }
+  if (v.kernel == TSLB_KERNEL_TILED) {
+    std::string why;
+    if (!tiled_plan_create(c->tiled, p->precision, v.L, c->fields, v.nfields, p->device, why)) {
+      g_create_error = "tiled kernel set-up failed: " + why;
+      if (c->own_ws) cudaFree(c->ws);
+      delete c;
+      return TSLB_ECUDA;
+    }
+    c->kname = c->tiled.name;
+  } else {
+    c->kname = "generic";
+  }
+  *out = c;
+  return TSLB_OK;
+}
+
+int tslb_init_fields(tslb_ctx *c, const void *rho, const void *ux, const void *uy, const void *uz,
+                     const void *phi, const void *const pineq[6], int pointers_on_device) {
+  if (!c) return TSLB_EINVAL;
+  if (!rho || !ux || !uy || !uz) return c->fail(TSLB_EINVAL, "rho, ux, uy, uz are required");
+  if (c->p.two_component && !phi) return c->fail(TSLB_EINVAL, "phi is required when two_component");
+  if (!c->p.two_component && phi) return c->fail(TSLB_EINVAL, "phi must be NULL when !two_component");
+  CK(cudaSetDevice(c->p.device));
+  const size_t N = (size_t)c->p.nx * c->p.ny * c->p.nz;
+  if (!pointers_on_device && !c->stage) {
+    cudaError_t e = cudaMalloc(&c->stage, N * c->v.esize);
+    if (e != cudaSuccess) return c->fail(TSLB_ENOMEM, "cudaMalloc(stage): %s", cudaGetErrorString(e));
+  }
+  const void *src[NF_MAX] = {rho, ux, uy, uz, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, phi};
+  if (pineq)
+    for (int k = 0; k < 6; ++k) src[F_PXX + k] = pineq[k];
+  int rc = c->p.precision == TSLB_F32 ? init_typed<float>(c, src, pointers_on_device)
+                                      : init_typed<double>(c, src, pointers_on_device);
+  if (rc == TSLB_OK) c->inited = true;
+  return rc;
+}
+
+int tslb_step(tslb_ctx *c, int nsteps) {
+  if (!c) return TSLB_EINVAL;
+  if (nsteps < 0) return c->fail(TSLB_EINVAL, "nsteps must be >= 0");
+  if (!c->inited) return c->fail(TSLB_ESTATE, "tslb_step before tslb_init_fields");
+  CK(cudaSetDevice(c->p.device));
+  return c->p.precision == TSLB_F32 ? step_typed<float>(c, nsteps) : step_typed<double>(c, nsteps);
+}
+
+int tslb_get_moments(tslb_ctx *c, void *rho, void *ux, void *uy, void *uz, void *const pineq[6],
+                     void *phi, int pointers_on_device) {
+  if (!c) return TSLB_EINVAL;
+  if (!c->inited) return c->fail(TSLB_ESTATE, "tslb_get_moments before tslb_init_fields");
+  if (phi && !c->p.two_component) return c->fail(TSLB_EINVAL, "phi requested from a single-component context");
+  CK(cudaSetDevice(c->p.device));
+  const size_t N = (size_t)c->p.nx * c->p.ny * c->p.nz;
+  if (!pointers_on_device && !c->stage) {
+    cudaError_t e = cudaMalloc(&c->stage, N * c->v.esize);
+    if (e != cudaSuccess) return c->fail(TSLB_ENOMEM, "cudaMalloc(stage): %s", cudaGetErrorString(e));
+  }
+  void *dst[NF_MAX] = {rho, ux, uy, uz, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, phi};
+  if (pineq)
+    for (int k = 0; k < 6; ++k) dst[F_PXX + k] = pineq[k];
+  return c->p.precision == TSLB_F32 ? get_typed<float>(c, dst, pointers_on_device)
+                                    : get_typed<double>(c, dst, pointers_on_device);
+}
+
+long long tslb_step_count(const tslb_ctx *c) { return c ? c->t : -1; }
+const char *tslb_kernel_name(const tslb_ctx *c) { return c ? c->kname.c_str() : ""; }
+long long tslb_launch_count(const tslb_ctx *c) { return c ? c->launches : -1; }
+
+int tslb_debug_xi(tslb_ctx *c, long long step, double *out_host) {
+  if (!c || !out_host) return TSLB_EINVAL;
+  CK(cudaSetDevice(c->p.device));
+  const int nx = c->p.nx, ny = c->p.ny;
+  double *d = nullptr;
+  CK(cudaMalloc(&d, sizeof(double) * nx * ny));
+  dim3 b(128), g((nx + 127) / 128, ny);
+  if (c->p.precision == TSLB_F32) debug_xi_kernel<float><<<g, b, 0, c->stream>>>(c->p.seed, nx, ny, step, d);
+  else debug_xi_kernel<double><<<g, b, 0, c->stream>>>(c->p.seed, nx, ny, step, d);
+  cudaError_t e = cudaMemcpyAsync(out_host, d, sizeof(double) * nx * ny, cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  cudaFree(d);
+  if (e != cudaSuccess) return c->cuda_fail(e, "tslb_debug_xi");
+  return TSLB_OK;
+}
+
+int tslb_destroy(tslb_ctx *c) {
+  if (!c) return TSLB_OK;
+  cudaSetDevice(c->p.device);
+  cudaStreamSynchronize(c->stream);
+  tiled_plan_destroy(c->tiled);
+  if (c->stage) cudaFree(c->stage);
+  if (c->own_ws && c->ws) cudaFree(c->ws);
+  delete c;
+  return TSLB_OK;
+}
+
+const char *tslb_last_error(const tslb_ctx *c) { return c ? c->err.c_str() : g_create_error.c_str(); }
+
+}  // extern "C"
