@@ -16,6 +16,7 @@
 // moment lives in the order-0 term (reading A17).
 #pragma once
 #include "tslb_common.cuh"
+#include "tslb_pair.cuh"
 
 namespace tslb {
 
@@ -61,6 +62,34 @@ __device__ __forceinline__ void post_collision_coeffs(V drho, V ux, V uy, V uz, 
     Kt[K111] = V(27) * (axy * uz + qxz * uy + qyz * ux);
   } else {
     Kt[K210] = Kt[K201] = Kt[K120] = Kt[K021] = Kt[K102] = Kt[K012] = Kt[K111] = V(0);
+  }
+}
+
+// Un-normalised Hermite coefficients K_abc (same 17, same order) with explicit FMAs, for the
+// tiled kernel where V is a packed pair; the 1/norm factors are folded into the 1-D operators.
+template <int ORDER, typename V>
+__device__ __forceinline__ void hermite_coeffs(V drho, V ux, V uy, V uz, V pxx, V pyy, V pzz, V pxy, V pxz,
+                                               V pyz, V omc, V *K) {
+  const V rho = drho + V(1);
+  const V mx = rho * ux, my = rho * uy, mz = rho * uz;
+  const V qxy = omc * pxy, qxz = omc * pxz, qyz = omc * pyz;
+  const V axx = pfma(mx, ux, omc * pxx), ayy = pfma(my, uy, omc * pyy), azz = pfma(mz, uz, omc * pzz);
+  const V axy = pfma(mx, uy, qxy), axz = pfma(mx, uz, qxz), ayz = pfma(my, uz, qyz);
+  K[K000] = drho;
+  K[K100] = mx; K[K010] = my; K[K001] = mz;
+  K[K200] = axx; K[K020] = ayy; K[K002] = azz;
+  K[K110] = axy; K[K101] = axz; K[K011] = ayz;
+  if (ORDER >= 3) {
+    const V txy = qxy + qxy, txz = qxz + qxz, tyz = qyz + qyz;
+    K[K210] = pfma(txy, ux, axx * uy);
+    K[K201] = pfma(txz, ux, axx * uz);
+    K[K120] = pfma(txy, uy, ayy * ux);
+    K[K021] = pfma(tyz, uy, ayy * uz);
+    K[K102] = pfma(txz, uz, azz * ux);
+    K[K012] = pfma(tyz, uz, azz * uy);
+    K[K111] = pfma(qyz, ux, pfma(qxz, uy, axy * uz));
+  } else {
+    K[K210] = K[K201] = K[K120] = K[K021] = K[K102] = K[K012] = K[K111] = V(0);
   }
 }
 

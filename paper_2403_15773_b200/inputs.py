@@ -163,7 +163,7 @@ def jet_developed(nx, ny, nz, D, U=0.05, seed=99, ndrop=200, W=4.0):
     core = 0.5 * (1.0 - np.tanh(2.0 * (r - D / 2.0) / W)) * (zz < nz / 3.0)
     phi = core
     for _ in range(ndrop):
-        cz = rng.uniform(nz / 3.0, nz - 8.0)
+        cz = rng.uniform(nz / 3.0, max(nz / 3.0 + 1.0, nz - 8.0))
         spread = 0.1 * (cz + z0)
         cx, cy = rng.normal(0, spread, 2)
         rad = rng.uniform(3.0, 0.2 * D + 3.0)

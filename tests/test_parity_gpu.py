@@ -281,6 +281,8 @@ def test_ragged_grids_generic(precision, shape):
     nx, ny, nz = shape
     prm = dict(nx=nx, ny=ny, nz=nz, omega=1.7, two_component=True, sigma=0.01, interface_width=3.0)
     steps = 20 if precision == tslb.F64 else 10
+    if nx * ny * nz < 64:
+        steps = 5          # a 1-node periodic box only relaxes Pi^neq -> (1-omega)^t Pi^neq: keep it O(1)
     check("rag%s" % (shape,), lambda: inputs.smooth_random(nx, ny, nz, seed=nx + ny), prm, steps, precision,
           tslb.KERNEL_GENERIC)
 
