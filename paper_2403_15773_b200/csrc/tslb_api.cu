@@ -166,7 +166,7 @@ int step_typed(tslb_ctx *c, int nsteps) {
     int rc;
     if (c->v.kernel == TSLB_KERNEL_TILED) {
       cudaError_t e = launch_tiled<T>(c->tiled, P, c->cur, c->p.hermite_order, c->p.two_component != 0, c->stream);
-      c->launches++;
+      c->launches += c->v.zper ? 1 : 2;   // + the boundary-plane kernel with inflow/outflow
       rc = (e == cudaSuccess) ? TSLB_OK : c->cuda_fail(e, "launch_tiled");
     } else {
       rc = launch_generic<T>(c, P);
