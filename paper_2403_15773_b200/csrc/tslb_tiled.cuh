@@ -9,15 +9,17 @@
 // The 27-neighbour pull of PAPER.md:98 eq. 6 / Fig. 1 is evaluated in the tensor-product Hermite
 // basis (tslb_math.cuh) as three 1-D three-point passes:
 //   x-pass  (segment 1)  K_abc (17 per node, recomputed for the pair's two x-neighbours)
-//                        -> X^p_bc (24 per node), written to shared memory for tile rows +-1;
-//   y-pass  (segment 2)  X^p_bc at rows y-1,y,y+1 -> Y^pq_c (18, registers);
+//                        -> X^p_bc (24 per node, registers);
+//   y-push  (seg. 1->2)  every row forms, per (p,c), the combination a+ it sends to the row above,
+//                        a- it sends to the row below and a0 it keeps: only 9+9 values per node
+//                        cross shared memory (not 24 x 3 rows) -> Y^pq_c (18, registers);
 //   z-push  (segment 2)  Y^pq_c of source plane k is pushed into the register accumulators of
 //                        the destination planes k-1, k, k+1 (two live accumulator sets);
 // so each stored moment is read from HBM once and the populations never exist in memory.
 // The phase-field half (eqs. 20-24) runs in the same kernel from the phi ring:
-// z-combinations of phi (aux warps), G and n = G/(|G|+eps) on tile+1 into a 3-plane ring,
-// kappa = -div n, the kick, and the D3Q7 update assembled from per-plane fluxes -- phi, grad(phi),
-// n and kappa never touch HBM.
+// y-z pre-combinations T,U,V of phi (aux warps), G and n = G/(|G|+eps) on tile+1 into a 3-plane
+// ring, z-combinations of n, kappa = -div n, the kick, and the D3Q7 update assembled from
+// per-plane fluxes -- phi, grad(phi), n and kappa never touch HBM.
 //
 // Thread roles: TY "compute" rows own the tile; 2 "aux" rows do the x-pass of the two halo rows,
 // the phi z-combinations and the ring of the n field.  Two __syncthreads per plane.
@@ -71,30 +73,29 @@ struct TileCfg {
   // (16-byte-odd rows raised "illegal instruction" on B200), so fp32 stages 4.
   static constexpr int HL = sizeof(T) == 4 ? 4 : 2;
   static constexpr int RX = TX + 2 * HL;   // staged columns x0-HL .. x0+TX+HL-1
-  static constexpr int RY = TY + 2;        // staged moment rows y0-1 .. y0+TY
+  static constexpr int RY = TY + 2;        // staged moment rows y0-1 .. y0+TY   ("region rows")
   static constexpr int RYP = TY + 4;       // staged phi rows y0-2 .. y0+TY+1
   static constexpr int S = 3;              // moment ring (planes k-1, k, k+1)
   static constexpr int SP = 4;             // phi ring
-  static constexpr int NR = 3;             // ring of n / |G| planes
+  static constexpr int NR = 3;             // ring of n planes
   static constexpr int NTHREADS = LX * RY;
   static constexpr int NAUX = 2 * LX;
-  static constexpr int NX = 24;            // x-pass outputs per node
+  static constexpr int NYP = 9;            // y-push fields per direction: (p,c)
   static constexpr size_t al(size_t b) { return (b + 127) / 128 * 128; }
   static constexpr size_t MOM_BYTES = (size_t)10 * RY * RX * sizeof(T);   // one TMA box
   static constexpr size_t PHI_BYTES = (size_t)RYP * RX * sizeof(T);
   static constexpr size_t MOM_STAGE = al(MOM_BYTES);
   static constexpr size_t PHI_STAGE = al(PHI_BYTES);
+  static constexpr size_t PLANE = al((size_t)RY * RX * sizeof(T));        // one region-plane array
+  static constexpr size_t YP_FIELD = al((size_t)RY * TX * sizeof(T));
   static constexpr size_t OFF_MOM = 0;
   static constexpr size_t OFF_PHI = OFF_MOM + S * MOM_STAGE;
-  static constexpr size_t OFF_SZ = OFF_PHI + (TWO ? SP * PHI_STAGE : 0);
-  static constexpr size_t OFF_DZ = OFF_SZ + (TWO ? PHI_STAGE : 0);
-  static constexpr size_t NRM_PLANE = al((size_t)RY * RX * sizeof(T));
-  static constexpr size_t OFF_NRM = OFF_DZ + (TWO ? PHI_STAGE : 0);
-  static constexpr size_t GM_PLANE = al((size_t)TY * TX * sizeof(T));
-  static constexpr size_t OFF_GM = OFF_NRM + (TWO ? NR * 3 * NRM_PLANE : 0);
-  static constexpr size_t X_FIELD = al((size_t)RY * TX * sizeof(T));
-  static constexpr size_t OFF_X = OFF_GM + (TWO ? NR * GM_PLANE : 0);
-  static constexpr size_t OFF_BAR = OFF_X + NX * X_FIELD;
+  static constexpr size_t OFF_TUV = OFF_PHI + (TWO ? SP * PHI_STAGE : 0);  // T, U, V of plane k
+  static constexpr size_t OFF_NRM = OFF_TUV + (TWO ? 3 * PLANE : 0);       // n ring [NR][3]
+  static constexpr size_t OFF_ZC = OFF_NRM + (TWO ? NR * 3 * PLANE : 0);   // S_z n_x, S_z n_y, d_z n_z
+  static constexpr size_t OFF_AP = OFF_ZC + (TWO ? 3 * PLANE : 0);         // y-push, upward  [9]
+  static constexpr size_t OFF_AM = OFF_AP + NYP * YP_FIELD;                // y-push, downward [9]
+  static constexpr size_t OFF_BAR = OFF_AM + NYP * YP_FIELD;
   static constexpr size_t SMEM_BYTES = OFF_BAR + 64;
 };
 
@@ -105,31 +106,49 @@ struct TiledMaps {
   int zc;            // planes per z chunk
 };
 
-// 1-D three-point operators of the tensor-product basis, un-normalised input coefficient of
-// Hermite index U, output moment of Hermite index W, acting on P = g(-1)+g(+1) side sums
-// (P = g(x-1)+g(x+1), Q = g(x-1)-g(x+1), C = g(x)); table derived in DESIGN.md §6:
-//   U=0: W0: P/6+2C/3   W1: Q/6   W2: P/9-2C/9
-//   U=1: W0: Q/2        W1: P/2   W2: Q/3
-//   U=2: W0: P/2-C      W1: Q/2   W2: (P+C)/3
-template <int U, int W, typename V, typename T>
-__device__ __forceinline__ V op_acc(V acc, V Pv, V Qv, V Cv) {
-  if (U == 0 && W == 0) return pfma(Cv, T(2.0 / 3.0), pfma(Pv, T(1.0 / 6.0), acc));
-  if (U == 0 && W == 1) return pfma(Qv, T(1.0 / 6.0), acc);
-  if (U == 0 && W == 2) return pfma(Cv, T(-2.0 / 9.0), pfma(Pv, T(1.0 / 9.0), acc));
-  if (U == 1 && W == 0) return pfma(Qv, T(0.5), acc);
-  if (U == 1 && W == 1) return pfma(Pv, T(0.5), acc);
-  if (U == 1 && W == 2) return pfma(Qv, T(1.0 / 3.0), acc);
-  if (U == 2 && W == 0) return pfma(Pv, T(0.5), acc - Cv);
-  if (U == 2 && W == 1) return pfma(Qv, T(0.5), acc);
-  return pfma(Pv + Cv, T(1.0 / 3.0), acc);
-}
-
 template <typename T> __device__ __forceinline__ Pair<T> prcp(Pair<T> a);
 template <> __device__ __forceinline__ F2 prcp<float>(F2 a) { return F2(__frcp_rn(a.x), __frcp_rn(a.y)); }
 template <> __device__ __forceinline__ D2 prcp<double>(D2 a) { return D2(1.0 / a.x, 1.0 / a.y); }
-
 __device__ __forceinline__ float rcp1(float s) { return __frcp_rn(s); }
 __device__ __forceinline__ double rcp1(double s) { return 1.0 / s; }
+
+// The 1-D three-point operator of the tensor-product basis in PUSH form.  A source
+// node holding the un-normalised Hermite coefficients g_0, g_1, g_2 (index along this axis) sends
+//     a+ = g0/6 + g1/2 + g2/2   to the node at +1,
+//     a- = g0/6 - g1/2 + g2/2   to the node at -1,  and keeps  a0 = 2 g0/3 - g2;
+// the destination's Hermite moments along the axis are then
+//     W0 = a+(-1) + a0 + a-(+1),   W1 = a+(-1) - a-(+1),   W2 = 2/3 (a+(-1) + a-(+1)) - a0/3.
+// (w(+-1) = 1/6, w(0) = 2/3, norms 1, 1/3, 2/9: a+ = w h_a(+1)/norm_a summed over a, etc.)
+template <int NA, typename V, typename T>
+__device__ __forceinline__ void push3(V g0, V g1, V g2, V &ap, V &am, V &a0) {
+  V h = g0 * T(1.0 / 6.0);
+  if (NA == 3) h = pfma(g2, T(0.5), h);
+  ap = h; am = h;
+  if (NA >= 2) { ap = pfma(g1, T(0.5), h); am = pfma(g1, T(-0.5), h); }
+  a0 = g0 * T(2.0 / 3.0);
+  if (NA == 3) a0 = a0 - g2;
+}
+// destination side: from up = a+(-1), dn = a-(+1), a0 -> W0, W1, W2
+template <typename V, typename T>
+__device__ __forceinline__ void pull3(V up, V dn, V a0, V &W0, V &W1, V &W2) {
+  const V s = up + dn;
+  W0 = s + a0;
+  W1 = up - dn;
+  W2 = pfma(s, T(2.0 / 3.0), a0 * T(-1.0 / 3.0));
+}
+
+// x-pass of one (b,c) group for the node pair (x, x+1) from the coefficients on the shifted pairs
+// A = (x-1, x) and B = (x+1, x+2): a+ is needed at A, a- at B and a0 at (A.y, B.x).
+template <int NA, typename V, typename T>
+__device__ __forceinline__ void xgroup(const V *KA, const V *KB, int i0, int i1, int i2, V &X0, V &X1, V &X2) {
+  V hA = KA[i0] * T(1.0 / 6.0), hB = KB[i0] * T(1.0 / 6.0);
+  if (NA == 3) { hA = pfma(KA[i2], T(0.5), hA); hB = pfma(KB[i2], T(0.5), hB); }
+  V ap = hA, am = hB;
+  if (NA >= 2) { ap = pfma(KA[i1], T(0.5), hA); am = pfma(KB[i1], T(-0.5), hB); }
+  V a0(T(2.0 / 3.0) * KA[i0].y, T(2.0 / 3.0) * KB[i0].x);
+  if (NA == 3) { a0.x -= KA[i2].y; a0.y -= KB[i2].x; }
+  pull3<V, T>(ap, am, a0, X0, X1, X2);
+}
 
 // ------------------------------------------------------------------ the kernel
 template <typename T, int TX, int TY, int ORDER, bool TWO>
@@ -138,15 +157,18 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   using C = TileCfg<T, TX, TY, TWO>;
   using V = Pair<T>;
   constexpr int LX = C::LX, HL = C::HL, RX = C::RX, RY = C::RY, RYP = C::RYP, S = C::S, SP = C::SP, NR = C::NR;
+  constexpr int PL = (int)(C::PLANE / sizeof(T));       // elements per region-plane array
+  constexpr int YPF = (int)(C::YP_FIELD / sizeof(T));   // elements per y-push field
+  constexpr int MF = RY * RX;                           // elements per moment field in a stage
   extern __shared__ __align__(128) unsigned char smem[];
   uint64_t *bars = reinterpret_cast<uint64_t *>(smem + C::OFF_BAR);
-  auto mom_at = [&](int slot, int f) { return reinterpret_cast<T *>(smem + C::OFF_MOM + slot * C::MOM_STAGE) + (size_t)f * RY * RX; };
+  auto mom_at = [&](int slot) { return reinterpret_cast<T *>(smem + C::OFF_MOM + slot * C::MOM_STAGE); };
   auto phi_at = [&](int slot) { return reinterpret_cast<T *>(smem + C::OFF_PHI + slot * C::PHI_STAGE); };
-  auto nrm_at = [&](int slot, int comp) { return reinterpret_cast<T *>(smem + C::OFF_NRM + (slot * 3 + comp) * C::NRM_PLANE); };
-  auto gm_at = [&](int slot) { return reinterpret_cast<T *>(smem + C::OFF_GM + slot * C::GM_PLANE); };
-  auto x_at = [&](int f) { return reinterpret_cast<T *>(smem + C::OFF_X + f * C::X_FIELD); };
-  T *s_sz = reinterpret_cast<T *>(smem + C::OFF_SZ);
-  T *s_dz = reinterpret_cast<T *>(smem + C::OFF_DZ);
+  auto nrm_at = [&](int slot) { return reinterpret_cast<T *>(smem + C::OFF_NRM + slot * 3 * C::PLANE); };
+  T *s_tuv = reinterpret_cast<T *>(smem + C::OFF_TUV);
+  T *s_zc = reinterpret_cast<T *>(smem + C::OFF_ZC);
+  T *s_ap = reinterpret_cast<T *>(smem + C::OFF_AP);
+  T *s_am = reinterpret_cast<T *>(smem + C::OFF_AM);
 
   const Layout &L = P.L;
   const int t = threadIdx.x;
@@ -154,7 +176,10 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   const int tr = t / LX;
   const bool aux = tr >= TY;
   const int r = aux ? (tr == TY ? 0 : RY - 1) : tr + 1;   // region row (y = y0 - 1 + r)
-  const int c0 = HL + 2 * lx;                              // staged column of the pair's first node
+  const int c0 = HL + 2 * lx;                             // staged column of the pair's first node
+  const int oM = r * RX + c0;                             // offset of the pair in a region plane
+  const int oY = r * TX + 2 * lx;                         // offset of the pair in a y-push field
+  const int ia = (tr - TY) * LX + lx;                     // aux thread index
   const int x0 = (blockIdx.x % M.ntx) * TX;
   const int y0 = (blockIdx.x / M.ntx) * TY;
   const int z0 = blockIdx.y * M.zc;
@@ -173,7 +198,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     uint32_t bytes = (uint32_t)C::MOM_BYTES + (TWO ? (uint32_t)C::PHI_BYTES : 0u);
     if (TWO && g == 0) bytes += 2u * (uint32_t)C::PHI_BYTES;
     mbar_expect_tx(bar, bytes);
-    tma_load_4d(mom_at(g % S, 0), &M.mom, bar, x0 - HL + GX, y0 - 1 + GY, zmap(kb + g), 0);
+    tma_load_4d(mom_at(g % S), &M.mom, bar, x0 - HL + GX, y0 - 1 + GY, zmap(kb + g), 0);
     if (TWO) {
       tma_load_3d(phi_at((g + 2) % SP), &M.phi, bar, x0 - HL + GX, y0 - 2 + GY, zmap(kb + g + 1));
       if (g == 0) {
@@ -183,85 +208,113 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     }
   };
 
-#if defined(TSLB_DBG) && TSLB_DBG == 5
-  return;
-#endif
   if (t == 0) {
     for (int s = 0; s < S; ++s) mbar_init(&bars[s], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
   __syncthreads();
-#if defined(TSLB_DBG) && TSLB_DBG == 4
-  return;
-#endif
   if (t == 0) {
     issue(0);
     if (NG > 1) issue(1);
   }
 
   const V omc(P.omc);
+  const T w1 = T(1.0 / 6.0), w0 = T(2.0 / 3.0);
   V accA[10], accB[10];     // Hermite moments being accumulated for planes k and k+1
   V fl[10];                 // finished flow part of the plane completed in the previous iteration:
                             // drho', u_b (3), Pi^neq' (6)
+  V A0[9];                  // this row's own y-push term a0 per (c,p), carried across the barrier
+  V nA[3], nB[3];           // own n of planes k-2 and k-1
+  V gA(T(0)), gB(T(0));     // own |G| of planes k-2 and k-1
   V c_inpl(T(0)), c_upa(T(0)), c_upb(T(0));
 #pragma unroll
   for (int m = 0; m < 10; ++m) { accA[m] = V(T(0)); accB[m] = V(T(0)); fl[m] = V(T(0)); }
+#pragma unroll
+  for (int m = 0; m < 3; ++m) { nA[m] = V(T(0)); nB[m] = V(T(0)); }
 
+  // global store offsets of the pair (plane 0); the periodic ghost images of edge nodes
+  const int gx_ = x0 + 2 * lx, gy_ = y0 + tr;
+  const int gxg = gx_ < 2 ? gx_ + L.nx : (gx_ >= L.nx - 2 ? gx_ - L.nx : gx_);
+  const int gyg = gy_ < GY ? gy_ + L.ny : (gy_ >= L.ny - GY ? gy_ - L.ny : gy_);
+  const long long o00 = L.idx(gx_, gy_, 0), o10 = L.idx(gxg, gy_, 0), o01 = L.idx(gx_, gyg, 0), o11 = L.idx(gxg, gyg, 0);
+
+  int ms = 0, ps = 0, ns = 0;   // ring slots of this iteration: moments i%S, phi(k-1) i%SP, n(k) i%NR
   for (int i = 0; i < NI; ++i) {
     const int k = kb + i;
-#if defined(TSLB_DBG) && TSLB_DBG == 1
-    return;
-#endif
-    if (i < NG) mbar_wait(&bars[i % S], (uint32_t)((i / S) & 1));
-#if defined(TSLB_DBG) && TSLB_DBG == 2
-    __syncthreads(); return;
-#endif
+    if (i < NG) mbar_wait(&bars[ms], (uint32_t)((i / S) & 1));
+    const int ms1 = ms == 0 ? S - 1 : ms - 1;          // moments of plane k-1
+    const int ns1 = ns == 0 ? NR - 1 : ns - 1;         // n of plane k-1
+    const int ns2 = ns1 == 0 ? NR - 1 : ns1 - 1;       // n of plane k-2
+    const T *phm = phi_at(ps);                         // phi(k-1)
+    const T *phc = phi_at((ps + 1) % SP);              // phi(k)
+    const T *php = phi_at((ps + 2) % SP);              // phi(k+1)
 
     // =========================== segment 1 ===========================
     if (TWO && aux && i < NG) {
-      // A1: z-combinations of phi for plane k: sz = S_z phi, dz = delta_z phi on the phi halo region
-      const T *pm = phi_at(i % SP), *pc = phi_at((i + 1) % SP), *pp = phi_at((i + 2) % SP);
-      const int ia = (tr - TY) * LX + lx;
-      for (int e = ia; e < RYP * RX / 2; e += C::NAUX) {
-        const V a = lds_pair(pm + 2 * e), b = lds_pair(pc + 2 * e), c = lds_pair(pp + 2 * e);
-        sts_pair(s_sz + 2 * e, pfma(b, T(2.0 / 3.0), (a + c) * T(1.0 / 6.0)));
-        sts_pair(s_dz + 2 * e, (c - a) * T(0.5));
+      // A1: T = S_y S_z phi, U = d_y S_z phi, V = S_y d_z phi of plane k on the region rows
+      for (int e = ia; e < RY * (RX / 2); e += C::NAUX) {
+        const int rr = e / (RX / 2), cp = 2 * (e - rr * (RX / 2));
+        const int o = (rr + 1) * RX + cp;
+        V sz[3], dz[3];
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+          const V a = lds_pair(phm + o + (d - 1) * RX), b = lds_pair(phc + o + (d - 1) * RX), c = lds_pair(php + o + (d - 1) * RX);
+          sz[d] = pfma(b, w0, (a + c) * w1);
+          dz[d] = (c - a) * T(0.5);
+        }
+        sts_pair(s_tuv + rr * RX + cp, pfma(sz[1], w0, (sz[0] + sz[2]) * w1));
+        sts_pair(s_tuv + PL + rr * RX + cp, (sz[2] - sz[0]) * T(0.5));
+        sts_pair(s_tuv + 2 * PL + rr * RX + cp, pfma(dz[1], w0, (dz[0] + dz[2]) * w1));
       }
     }
     if (i < NG) {
-      // A2: x-pass of region row r of plane k.  A = nodes (x-1, x), B = nodes (x+1, x+2).
+      // A2: x-pass of region row r of plane k, then the y-push terms.  A = nodes (x-1, x), B = (x+1, x+2).
       V KA[NK], KB[NK];
       {
         V mA[10], mB[10];
+        const T *p = mom_at(ms) + oM;
 #pragma unroll
         for (int f = 0; f < 10; ++f) {
-          const T *p = mom_at(i % S, f) + r * RX + c0;
-          const V own = lds_pair(p);
-          mA[f] = V(p[-1], own.x);
-          mB[f] = V(own.y, p[2]);
+          const V own = lds_pair(p + f * MF);
+          mA[f] = V(p[f * MF - 1], own.x);
+          mB[f] = V(own.y, p[f * MF + 2]);
         }
         hermite_coeffs<ORDER, V>(mA[0], mA[1], mA[2], mA[3], mA[4], mA[5], mA[6], mA[7], mA[8], mA[9], omc, KA);
         hermite_coeffs<ORDER, V>(mB[0], mB[1], mB[2], mB[3], mB[4], mB[5], mB[6], mB[7], mB[8], mB[9], omc, KB);
       }
-      // groups (b,c) -> K indices for a = 0,1,2 (-1: absent)
-      constexpr int GA[8][3] = {{K000, K100, K200}, {K010, K110, K210}, {K001, K101, K201}, {K020, K120, -1},
-                                {K002, K102, -1},   {K011, K111, -1},   {K021, -1, -1},     {K012, -1, -1}};
+      V Xb[3][3];   // [b][p] of the current c
+      // c = 0: groups (b,c) = (0,0) a=0,1,2 | (1,0) a=0,1,2 | (2,0) a=0,1
+      xgroup<3, V, T>(KA, KB, K000, K100, K200, Xb[0][0], Xb[0][1], Xb[0][2]);
+      xgroup<3, V, T>(KA, KB, K010, K110, K210, Xb[1][0], Xb[1][1], Xb[1][2]);
+      xgroup<2, V, T>(KA, KB, K020, K120, 0, Xb[2][0], Xb[2][1], Xb[2][2]);
 #pragma unroll
-      for (int g = 0; g < 8; ++g) {
-        V X0(T(0)), X1(T(0)), X2(T(0));
+      for (int p = 0; p < 3; ++p) {
+        V ap, am;
+        push3<3, V, T>(Xb[0][p], Xb[1][p], Xb[2][p], ap, am, A0[p]);
+        sts_pair(s_ap + p * YPF + oY, ap);
+        sts_pair(s_am + p * YPF + oY, am);
+      }
+      // c = 1: (0,1) a=0,1,2 | (1,1) a=0,1 | (2,1) a=0
+      xgroup<3, V, T>(KA, KB, K001, K101, K201, Xb[0][0], Xb[0][1], Xb[0][2]);
+      xgroup<2, V, T>(KA, KB, K011, K111, 0, Xb[1][0], Xb[1][1], Xb[1][2]);
+      xgroup<1, V, T>(KA, KB, K021, 0, 0, Xb[2][0], Xb[2][1], Xb[2][2]);
 #pragma unroll
-        for (int a = 0; a < 3; ++a) {
-          if (GA[g][a] < 0) continue;
-          const V ka = KA[GA[g][a]], kbv = KB[GA[g][a]];
-          const V Pv = ka + kbv, Qv = ka - kbv, Cv(ka.y, kbv.x);
-          if (a == 0) { X0 = op_acc<0, 0, V, T>(X0, Pv, Qv, Cv); X1 = op_acc<0, 1, V, T>(X1, Pv, Qv, Cv); X2 = op_acc<0, 2, V, T>(X2, Pv, Qv, Cv); }
-          if (a == 1) { X0 = op_acc<1, 0, V, T>(X0, Pv, Qv, Cv); X1 = op_acc<1, 1, V, T>(X1, Pv, Qv, Cv); X2 = op_acc<1, 2, V, T>(X2, Pv, Qv, Cv); }
-          if (a == 2) { X0 = op_acc<2, 0, V, T>(X0, Pv, Qv, Cv); X1 = op_acc<2, 1, V, T>(X1, Pv, Qv, Cv); X2 = op_acc<2, 2, V, T>(X2, Pv, Qv, Cv); }
-        }
-        sts_pair(x_at(3 * g + 0) + r * TX + 2 * lx, X0);
-        sts_pair(x_at(3 * g + 1) + r * TX + 2 * lx, X1);
-        sts_pair(x_at(3 * g + 2) + r * TX + 2 * lx, X2);
+      for (int p = 0; p < 3; ++p) {
+        V ap, am;
+        push3<3, V, T>(Xb[0][p], Xb[1][p], Xb[2][p], ap, am, A0[3 + p]);
+        sts_pair(s_ap + (3 + p) * YPF + oY, ap);
+        sts_pair(s_am + (3 + p) * YPF + oY, am);
+      }
+      // c = 2: (0,2) a=0,1 | (1,2) a=0
+      xgroup<2, V, T>(KA, KB, K002, K102, 0, Xb[0][0], Xb[0][1], Xb[0][2]);
+      xgroup<1, V, T>(KA, KB, K012, 0, 0, Xb[1][0], Xb[1][1], Xb[1][2]);
+#pragma unroll
+      for (int p = 0; p < 3; ++p) {
+        V ap, am;
+        push3<2, V, T>(Xb[0][p], Xb[1][p], Xb[1][p], ap, am, A0[6 + p]);
+        sts_pair(s_ap + (6 + p) * YPF + oY, ap);
+        sts_pair(s_am + (6 + p) * YPF + oY, am);
       }
     }
     if (!aux && i >= 1) {
@@ -269,126 +322,93 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
       const int j = k - 2;                         // plane finalised in this iteration
       const bool fin = (j >= z0);                  // (j < z1 always: k <= z1 + 1)
       if (TWO) {
-        // fluxes of plane k-1 (all operands resident: moments slot (i-1)%S, phi slot i%SP, n slot (i-1)%NR)
-        const int ms = (i - 1) % S, ns = (i - 1) % NR;
-        const T *ph = phi_at(i % SP) + (r + 1) * RX + c0;
+        // fluxes of plane k-1 (operands resident: moments slot ms1, phi(k-1) = phm, n(k-1) slot ns1)
+        const T *ph = phm + (r + 1) * RX + c0;
+        const T *mo = mom_at(ms1) + oM;
+        const T *nr = nrm_at(ns1) + oM;
         const T gam = P.gamma;
         auto gplus = [&](T p, T u, T n) { return p * (T(1) + T(4) * u) + gam * p * (T(1) - p) * n; };
         auto gminus = [&](T p, T u, T n) { return p * (T(1) - T(4) * u) - gam * p * (T(1) - p) * n; };
+        const V pc = lds_pair(ph);
         // x direction: columns c0-1 .. c0+2
-        const T *uxp = mom_at(ms, F_UX) + r * RX + c0;
-        const T *nxp = nrm_at(ns, 0) + r * RX + c0;
-        const V phc = lds_pair(ph), uxc = lds_pair(uxp), nxc = lds_pair(nxp);
+        const V uxc = lds_pair(mo + F_UX * MF);
         V inpl;
-        inpl.x = gplus(ph[-1], uxp[-1], nxp[-1]) + gminus(phc.y, uxc.y, nxc.y);
-        inpl.y = gplus(phc.x, uxc.x, nxc.x) + gminus(ph[2], uxp[2], nxp[2]);
+        inpl.x = gplus(ph[-1], mo[F_UX * MF - 1], nr[-1]) + gminus(pc.y, uxc.y, nB[0].y);
+        inpl.y = gplus(pc.x, uxc.x, nB[0].x) + gminus(ph[2], mo[F_UX * MF + 2], nr[2]);
         // y direction: rows r-1 (south, c_i = +e_y) and r+1 (north)
-        const T *uyp = mom_at(ms, F_UY) + r * RX + c0;
-        const T *nyp = nrm_at(ns, 1) + r * RX + c0;
-        const V phs = lds_pair(ph - RX), uys = lds_pair(uyp - RX), nys = lds_pair(nyp - RX);
-        const V phn_ = lds_pair(ph + RX), uyn = lds_pair(uyp + RX), nyn = lds_pair(nyp + RX);
+        const V phs = lds_pair(ph - RX), uys = lds_pair(mo + F_UY * MF - RX), nys = lds_pair(nr + PL - RX);
+        const V phn_ = lds_pair(ph + RX), uyn = lds_pair(mo + F_UY * MF + RX), nyn = lds_pair(nr + PL + RX);
         inpl.x += gplus(phs.x, uys.x, nys.x) + gminus(phn_.x, uyn.x, nyn.x);
         inpl.y += gplus(phs.y, uys.y, nys.y) + gminus(phn_.y, uyn.y, nyn.y);
-        inpl.x = T(0.25) * phc.x + T(0.125) * inpl.x;
-        inpl.y = T(0.25) * phc.y + T(0.125) * inpl.y;
+        inpl.x = T(0.25) * pc.x + T(0.125) * inpl.x;
+        inpl.y = T(0.25) * pc.y + T(0.125) * inpl.y;
         // z direction: this plane's contribution to the planes above (up) and below (down)
-        const V uzc = lds_pair(mom_at(ms, F_UZ) + r * RX + c0), nzc = lds_pair(nrm_at(ns, 2) + r * RX + c0);
-        const V up(gplus(phc.x, uzc.x, nzc.x), gplus(phc.y, uzc.y, nzc.y));
-        const V down(gminus(phc.x, uzc.x, nzc.x), gminus(phc.y, uzc.y, nzc.y));
+        const V uzc = lds_pair(mo + F_UZ * MF);
+        const V up(gplus(pc.x, uzc.x, nB[2].x), gplus(pc.y, uzc.y, nB[2].y));
+        const V down(gminus(pc.x, uzc.x, nB[2].x), gminus(pc.y, uzc.y, nB[2].y));
         if (fin) {
           // a7: phi'(j) = inpl(j) + up(j-1)/8 + down(j+1)/8       (eqs. 23-24)
           phin = pfma(c_upa + down, T(0.125), c_inpl);
-          // a5: kappa(j) = -div n over the 27-point stencil, n planes j-1, j, j+1
-          const int sm_ = (i + NR - 3) % NR, s0 = (i + NR - 2) % NR, sp_ = (i + NR - 1) % NR;
-          const T w1 = T(1.0 / 6.0), w0 = T(2.0 / 3.0);
-          V kap(T(0));
-          {
-            // d/dx of S_y S_z n_x
-            V own(T(0)), nb(T(0));
-            const int sl[3] = {sm_, s0, sp_};
+          // a5: kappa(j) = -div n from the z-combined normals a = S_z n_x, b = S_z n_y, c = d_z n_z
+          const T *za = s_zc + oM;
+          V own(T(0)), nb(T(0));
 #pragma unroll
-            for (int dz = 0; dz < 3; ++dz)
-#pragma unroll
-              for (int dy = -1; dy <= 1; ++dy) {
-                const T w = (dz == 1 ? w0 : w1) * (dy == 0 ? w0 : w1);
-                const T *q = nrm_at(sl[dz], 0) + (r + dy) * RX + c0;
-                own = pfma(lds_pair(q), w, own);
-                nb = pfma(V(q[-1], q[2]), w, nb);
-              }
-            kap.x += T(0.5) * (own.y - nb.x);
-            kap.y += T(0.5) * (nb.y - own.x);
-            // d/dy of S_x S_z n_y
-            V dO(T(0)), dN(T(0));
-#pragma unroll
-            for (int dz = 0; dz < 3; ++dz) {
-              const T w = (dz == 1 ? w0 : w1);
-              const T *qn = nrm_at(sl[dz], 1) + (r + 1) * RX + c0;
-              const T *qs = nrm_at(sl[dz], 1) + (r - 1) * RX + c0;
-              dO = pfma(lds_pair(qn) - lds_pair(qs), w, dO);
-              dN = pfma(V(qn[-1], qn[2]) - V(qs[-1], qs[2]), w, dN);
-            }
-            kap.x += T(0.5) * (w1 * dN.x + w0 * dO.x + w1 * dO.y);
-            kap.y += T(0.5) * (w1 * dO.x + w0 * dO.y + w1 * dN.y);
-            // d/dz of S_x S_y n_z
-            V eO(T(0)), eN(T(0));
-#pragma unroll
-            for (int dy = -1; dy <= 1; ++dy) {
-              const T w = (dy == 0 ? w0 : w1);
-              const T *qp = nrm_at(sp_, 2) + (r + dy) * RX + c0;
-              const T *qm = nrm_at(sm_, 2) + (r + dy) * RX + c0;
-              eO = pfma(lds_pair(qp) - lds_pair(qm), w, eO);
-              eN = pfma(V(qp[-1], qp[2]) - V(qm[-1], qm[2]), w, eN);
-            }
-            kap.x += T(0.5) * (w1 * eN.x + w0 * eO.x + w1 * eO.y);
-            kap.y += T(0.5) * (w1 * eO.x + w0 * eO.y + w1 * eN.y);
+          for (int dy = -1; dy <= 1; ++dy) {
+            const T w = dy == 0 ? w0 : w1;
+            own = pfma(lds_pair(za + dy * RX), w, own);
+            nb = pfma(V(za[dy * RX - 1], za[dy * RX + 2]), w, nb);
           }
-          // a6: F = sigma kappa G, G = n (|G| + eps); u' = u_b + F / rho'   (kappa = -div: sign below)
-          const V gm = lds_pair(gm_at(s0) + tr * TX + 2 * lx) + V(T(1e-12));
+          V kap(T(0.5) * (own.y - nb.x), T(0.5) * (nb.y - own.x));          // d/dx S_y a
+          const T *zb = za + PL;
+          const V dO = lds_pair(zb + RX) - lds_pair(zb - RX);
+          const V dN = V(zb[RX - 1], zb[RX + 2]) - V(zb[-RX - 1], zb[-RX + 2]);
+          kap.x += T(0.5) * (w1 * dN.x + w0 * dO.x + w1 * dO.y);            // S_x d/dy b
+          kap.y += T(0.5) * (w1 * dO.x + w0 * dO.y + w1 * dN.y);
+          const T *zc_ = za + 2 * PL;
+          V eO(T(0)), eN(T(0));
+#pragma unroll
+          for (int dy = -1; dy <= 1; ++dy) {
+            const T w = dy == 0 ? w0 : w1;
+            eO = pfma(lds_pair(zc_ + dy * RX), w, eO);
+            eN = pfma(V(zc_[dy * RX - 1], zc_[dy * RX + 2]), w, eN);
+          }
+          kap.x += w1 * eN.x + w0 * eO.x + w1 * eO.y;                        // S_x S_y c
+          kap.y += w1 * eO.x + w0 * eO.y + w1 * eN.y;
+          // a6: F = sigma kappa G, kappa = -div n, G = n (|G| + eps); u' = u_b + F / rho'
           const V rinv = prcp<T>(fl[0] + V(T(1)));
-          const V sc = (kap * gm) * rinv * (-P.sigma);
-          ukx = lds_pair(nrm_at(s0, 0) + r * RX + c0) * sc;
-          uky = lds_pair(nrm_at(s0, 1) + r * RX + c0) * sc;
-          ukz = lds_pair(nrm_at(s0, 2) + r * RX + c0) * sc;
+          const V sc = (kap * (gA + V(T(1e-12)))) * rinv * (-P.sigma);
+          ukx = nA[0] * sc; uky = nA[1] * sc; ukz = nA[2] * sc;
         }
         c_upa = c_upb; c_upb = up; c_inpl = inpl;
       }
       if (fin && (P.zper || (j > 0 && j < L.nz - 1))) {
         // a9: store plane j (and its periodic ghost images)
-        const int x = x0 + 2 * lx, y = y0 + tr;
         V o[NF_MAX];
         o[0] = fl[0];
         o[1] = fl[1] + ukx; o[2] = fl[2] + uky; o[3] = fl[3] + ukz;
 #pragma unroll
         for (int m = 4; m < 10; ++m) o[m] = fl[m];
         o[10] = phin;
-        const int xg = x < 2 ? x + L.nx : (x >= L.nx - 2 ? x - L.nx : x);
-        const int yg = y < GY ? y + L.ny : (y >= L.ny - GY ? y - L.ny : y);
-        const long long i00 = L.idx(x, y, j), i10 = L.idx(xg, y, j), i01 = L.idx(x, yg, j), i11 = L.idx(xg, yg, j);
+        const long long zo = (long long)j * L.plane;
 #pragma unroll
         for (int m = 0; m < (TWO ? 11 : 10); ++m) {
-          T *base = P.out.f[m];
-          *reinterpret_cast<V *>(base + i00) = o[m];
-          if (xg != x) *reinterpret_cast<V *>(base + i10) = o[m];
-          if (yg != y) {
-            *reinterpret_cast<V *>(base + i01) = o[m];
-            if (xg != x) *reinterpret_cast<V *>(base + i11) = o[m];
+          T *base = P.out.f[m] + zo;
+          *reinterpret_cast<V *>(base + o00) = o[m];
+          if (gxg != gx_) *reinterpret_cast<V *>(base + o10) = o[m];
+          if (gyg != gy_) {
+            *reinterpret_cast<V *>(base + o01) = o[m];
+            if (gxg != gx_) *reinterpret_cast<V *>(base + o11) = o[m];
           }
         }
       }
     }
     __syncthreads();
-#if defined(TSLB_DBG) && TSLB_DBG == 3
-    return;
-#endif
     if (t == 0 && i + 2 < NG) issue(i + 2);
 
     // =========================== segment 2 ===========================
     if (i < NG) {
       if (!aux) {
-        // B2: y-pass (rows r-1, r, r+1 of X) and z-push into the accumulators.
-        // X field of group (b,c) and x-moment p is 3*g + p with g as in GA above:
-        //   c = 0: b = 0,1,2 -> g = 0,1,3;  c = 1: b = 0,1,2 -> g = 2,5,6;  c = 2: b = 0,1 -> g = 4,7
-        constexpr int GB[3][3] = {{0, 1, 3}, {2, 5, 6}, {4, 7, -1}};
+        // B2: finish the y-pass (a+ from the row below, a- from the row above, own a0) and z-push.
         V outm[10];
 #pragma unroll
         for (int m = 0; m < 10; ++m) outm[m] = accA[m];
@@ -398,28 +418,15 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
         for (int p = 0; p < 3; ++p) {
           V Yq[3][3];   // [q][c]
 #pragma unroll
-          for (int q = 0; q < 3; ++q)
-#pragma unroll
-            for (int c = 0; c < 3; ++c) Yq[q][c] = V(T(0));
-#pragma unroll
-          for (int c = 0; c < 3; ++c)
-#pragma unroll
-            for (int b = 0; b < 3; ++b) {
-              if (GB[c][b] < 0) continue;
-              const T *xp = x_at(3 * GB[c][b] + p) + r * TX + 2 * lx;
-              const V gs = lds_pair(xp - TX), gc = lds_pair(xp), gn = lds_pair(xp + TX);
-              const V Pv = gs + gn, Qv = gs - gn;
-              if (b == 0) { Yq[0][c] = op_acc<0, 0, V, T>(Yq[0][c], Pv, Qv, gc); if (p <= 1) Yq[1][c] = op_acc<0, 1, V, T>(Yq[1][c], Pv, Qv, gc); if (p == 0) Yq[2][c] = op_acc<0, 2, V, T>(Yq[2][c], Pv, Qv, gc); }
-              if (b == 1) { Yq[0][c] = op_acc<1, 0, V, T>(Yq[0][c], Pv, Qv, gc); if (p <= 1) Yq[1][c] = op_acc<1, 1, V, T>(Yq[1][c], Pv, Qv, gc); if (p == 0) Yq[2][c] = op_acc<1, 2, V, T>(Yq[2][c], Pv, Qv, gc); }
-              if (b == 2) { Yq[0][c] = op_acc<2, 0, V, T>(Yq[0][c], Pv, Qv, gc); if (p <= 1) Yq[1][c] = op_acc<2, 1, V, T>(Yq[1][c], Pv, Qv, gc); if (p == 0) Yq[2][c] = op_acc<2, 2, V, T>(Yq[2][c], Pv, Qv, gc); }
-            }
+          for (int c = 0; c < 3; ++c) {
+            const V up = lds_pair(s_ap + (3 * c + p) * YPF + oY - TX);
+            const V dn = lds_pair(s_am + (3 * c + p) * YPF + oY + TX);
+            pull3<V, T>(up, dn, A0[3 * c + p], Yq[0][c], Yq[1][c], Yq[2][c]);
+          }
 #pragma unroll
           for (int q = 0; q + p <= 2; ++q) {
-            const V Y0 = Yq[q][0], Y1 = Yq[q][1], Y2 = Yq[q][2];
-            const V h = pfma(Y0, T(1.0 / 6.0), Y2 * T(0.5));
-            const V ap = pfma(Y1, T(0.5), h);      // -> plane k+1
-            const V am = pfma(Y1, T(-0.5), h);     // -> plane k-1
-            const V a0 = pfma(Y0, T(2.0 / 3.0), V(T(0)) - Y2);   // -> plane k
+            V ap, am, a0;
+            push3<3, V, T>(Yq[q][0], Yq[q][1], Yq[q][2], ap, am, a0);   // ap -> plane k+1, am -> plane k-1
             {
               const int m = MI[p][q][0];
               outm[m] = outm[m] + am; accA[m] = accB[m] + a0; accB[m] = ap;
@@ -448,53 +455,57 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
         fl[9] = outm[9] - outm[2] * fl[3];
       }
       if (TWO) {
-        // B1: G = grad(phi), n = G/(|G|+eps) of plane k on tile+1 -> ring slot i%NR
-        auto gn_pair = [&](int rr, int c, bool write_gm) {
-          // columns c-1 .. c+2 (clamped at the staged edge; edge results are never used)
-          const int cl = c > 0 ? c - 1 : 0, cr = c + 2 < RX ? c + 2 : RX - 1;
-          const int rp = rr + 1;
-          T Tc[4], Uc[4], Vc[4];
-#pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            const int cc = q == 0 ? cl : (q == 3 ? cr : c + q - 1);
-            const T s_m = s_sz[(rp - 1) * RX + cc], s_0 = s_sz[rp * RX + cc], s_p = s_sz[(rp + 1) * RX + cc];
-            const T d_m = s_dz[(rp - 1) * RX + cc], d_0 = s_dz[rp * RX + cc], d_p = s_dz[(rp + 1) * RX + cc];
-            Tc[q] = T(1.0 / 6.0) * (s_m + s_p) + T(2.0 / 3.0) * s_0;
-            Uc[q] = T(0.5) * (s_p - s_m);
-            Vc[q] = T(1.0 / 6.0) * (d_m + d_p) + T(2.0 / 3.0) * d_0;
-          }
-          T g[2][3];
-#pragma unroll
-          for (int e = 0; e < 2; ++e) {
-            g[e][0] = T(0.5) * (Tc[e + 2] - Tc[e]);
-            g[e][1] = T(1.0 / 6.0) * (Uc[e] + Uc[e + 2]) + T(2.0 / 3.0) * Uc[e + 1];
-            g[e][2] = T(1.0 / 6.0) * (Vc[e] + Vc[e + 2]) + T(2.0 / 3.0) * Vc[e + 1];
-          }
-          const T s0_ = g[0][0] * g[0][0] + g[0][1] * g[0][1] + g[0][2] * g[0][2];
-          const T s1_ = g[1][0] * g[1][0] + g[1][1] * g[1][1] + g[1][2] * g[1][2];
-          const T m0_ = tsqrt<T>(s0_), m1_ = tsqrt<T>(s1_);                    // |G|
-          const T i0_ = rcp1(m0_ + T(1e-12)), i1_ = rcp1(m1_ + T(1e-12));     // 1/(|G|+eps), reading A7
-          const int slot = i % NR;
-#pragma unroll
-          for (int a = 0; a < 3; ++a) sts_pair(nrm_at(slot, a) + rr * RX + c, V(g[0][a] * i0_, g[1][a] * i1_));
-          if (write_gm) sts_pair(gm_at(slot) + (rr - 1) * TX + (c - HL), V(m0_, m1_));
+        // B1: G = (d_x T, S_x U, S_x V), n = G/(|G|+eps) of plane k on tile+1 -> ring slot ns
+        T *nk = nrm_at(ns);
+        auto gn_pair = [&](int o, int ol, int orr, V nn[3], V &mag) {
+          const V tc = lds_pair(s_tuv + o), uc = lds_pair(s_tuv + PL + o), vc = lds_pair(s_tuv + 2 * PL + o);
+          const T tl = s_tuv[ol], tr_ = s_tuv[orr], ul = s_tuv[PL + ol], ur = s_tuv[PL + orr];
+          const T vl = s_tuv[2 * PL + ol], vr = s_tuv[2 * PL + orr];
+          const V gx(T(0.5) * (tc.y - tl), T(0.5) * (tr_ - tc.x));
+          const V gy(w1 * (ul + uc.y) + w0 * uc.x, w1 * (uc.x + ur) + w0 * uc.y);
+          const V gz(w1 * (vl + vc.y) + w0 * vc.x, w1 * (vc.x + vr) + w0 * vc.y);
+          const V s2 = pfma(gz, gz, pfma(gy, gy, gx * gx));
+          mag = V(tsqrt<T>(s2.x), tsqrt<T>(s2.y));                                  // |G|
+          const V inv(rcp1(mag.x + T(1e-12)), rcp1(mag.y + T(1e-12)));             // reading A7
+          nn[0] = gx * inv; nn[1] = gy * inv; nn[2] = gz * inv;
+          sts_pair(nk + o, nn[0]); sts_pair(nk + PL + o, nn[1]); sts_pair(nk + 2 * PL + o, nn[2]);
         };
         if (!aux) {
-          gn_pair(r, c0, true);
+          V nC[3], gC;
+          gn_pair(oM, oM - 1, oM + 2, nC, gC);
+          // z-combinations of the own normals for kappa(k-1)
+          sts_pair(s_zc + oM, pfma(nB[0], w0, (nA[0] + nC[0]) * w1));
+          sts_pair(s_zc + PL + oM, pfma(nB[1], w0, (nA[1] + nC[1]) * w1));
+          sts_pair(s_zc + 2 * PL + oM, (nC[2] - nA[2]) * T(0.5));
+#pragma unroll
+          for (int a = 0; a < 3; ++a) { nA[a] = nB[a]; nB[a] = nC[a]; }
+          gA = gB; gB = gC;
         } else {
-          const int ia = (tr - TY) * LX + lx;
           constexpr int PPR = TX / 2 + 2;                // pairs per full ring row: cols HL-2 .. HL+TX+1
           constexpr int NT = 2 * PPR + 2 * TY;           // ring tasks
+          const T *n1 = nrm_at(ns1), *n2 = nrm_at(ns2);
           for (int e = ia; e < NT; e += C::NAUX) {
             int rr, c;
             if (e < 2 * PPR) { rr = (e < PPR) ? 0 : RY - 1; c = HL - 2 + 2 * (e % PPR); }
             else { const int q = e - 2 * PPR; rr = 1 + (q >> 1); c = (q & 1) ? HL + TX : HL - 2; }
-            gn_pair(rr, c, false);
+            const int o = rr * RX + c;
+            const int ol = c > 0 ? o - 1 : o, orr = c + 2 < RX ? o + 2 : o + 1;   // clamped; edge results unused
+            V nC[3], gC;
+            gn_pair(o, ol, orr, nC, gC);
+            const V a2 = lds_pair(n2 + o), a1 = lds_pair(n1 + o);
+            const V b2 = lds_pair(n2 + PL + o), b1 = lds_pair(n1 + PL + o);
+            const V c2 = lds_pair(n2 + 2 * PL + o);
+            sts_pair(s_zc + o, pfma(a1, w0, (a2 + nC[0]) * w1));
+            sts_pair(s_zc + PL + o, pfma(b1, w0, (b2 + nC[1]) * w1));
+            sts_pair(s_zc + 2 * PL + o, (nC[2] - c2) * T(0.5));
           }
         }
       }
     }
     __syncthreads();
+    ms = ms == S - 1 ? 0 : ms + 1;
+    ps = ps == SP - 1 ? 0 : ps + 1;
+    ns = ns == NR - 1 ? 0 : ns + 1;
   }
 }
 
