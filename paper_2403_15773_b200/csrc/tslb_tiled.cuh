@@ -279,9 +279,8 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
         const T *p = mom_at(ms) + oM;
 #pragma unroll
         for (int f = 0; f < 10; ++f) {
-          const V own = lds_pair(p + f * MF);
-          mA[f] = V(p[f * MF - 1], own.x);
-          mB[f] = V(own.y, p[f * MF + 2]);
+          mA[f] = V(p[f * MF - 1], p[f * MF]);
+          mB[f] = V(p[f * MF + 1], p[f * MF + 2]);
         }
         hermite_coeffs<ORDER, V>(mA[0], mA[1], mA[2], mA[3], mA[4], mA[5], mA[6], mA[7], mA[8], mA[9], omc, KA);
         hermite_coeffs<ORDER, V>(mB[0], mB[1], mB[2], mB[3], mB[4], mB[5], mB[6], mB[7], mB[8], mB[9], omc, KB);
@@ -329,26 +328,25 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
         const T *ph = phm + (r + 1) * RX + c0;
         const T *mo = mom_at(ms1) + oM;
         const T *nr = nrm_at(ns1) + oM;
-        const T gam = P.gamma;
-        auto gplus = [&](T p, T u, T n) { return p * (T(1) + T(4) * u) + gam * p * (T(1) - p) * n; };
-        auto gminus = [&](T p, T u, T n) { return p * (T(1) - T(4) * u) - gam * p * (T(1) - p) * n; };
+        // q = phi (4 c.u + gamma (1-phi) c.n): the neighbour sends phi + q along +e, phi - q along -e
+        const V gamv(P.gamma);
+        auto qterm = [&](V p, V u, V n) { return p * pfma(pfma(p, V(T(0)) - gamv, gamv), n, u * T(4)); };
         const V pc = lds_pair(ph);
-        // x direction: columns c0-1 .. c0+2
+        // x direction: g+ at columns (c0-1, c0), g- at columns (c0+1, c0+2)
         const V uxc = lds_pair(mo + F_UX * MF);
-        V inpl;
-        inpl.x = gplus(ph[-1], mo[F_UX * MF - 1], nr[-1]) + gminus(pc.y, uxc.y, nB[0].y);
-        inpl.y = gplus(pc.x, uxc.x, nB[0].x) + gminus(ph[2], mo[F_UX * MF + 2], nr[2]);
+        const V pA(ph[-1], pc.x), pB(pc.y, ph[2]);
+        const V qA = qterm(pA, V(mo[F_UX * MF - 1], uxc.x), V(nr[-1], nB[0].x));
+        const V qB = qterm(pB, V(uxc.y, mo[F_UX * MF + 2]), V(nB[0].y, nr[2]));
+        V inpl = (pA + qA) + (pB - qB);
         // y direction: rows r-1 (south, c_i = +e_y) and r+1 (north)
-        const V phs = lds_pair(ph - RX), uys = lds_pair(mo + F_UY * MF - RX), nys = lds_pair(nr + PL - RX);
-        const V phn_ = lds_pair(ph + RX), uyn = lds_pair(mo + F_UY * MF + RX), nyn = lds_pair(nr + PL + RX);
-        inpl.x += gplus(phs.x, uys.x, nys.x) + gminus(phn_.x, uyn.x, nyn.x);
-        inpl.y += gplus(phs.y, uys.y, nys.y) + gminus(phn_.y, uyn.y, nyn.y);
-        inpl.x = T(0.25) * pc.x + T(0.125) * inpl.x;
-        inpl.y = T(0.25) * pc.y + T(0.125) * inpl.y;
+        const V phs = lds_pair(ph - RX), phn_ = lds_pair(ph + RX);
+        const V qS = qterm(phs, lds_pair(mo + F_UY * MF - RX), lds_pair(nr + PL - RX));
+        const V qN = qterm(phn_, lds_pair(mo + F_UY * MF + RX), lds_pair(nr + PL + RX));
+        inpl = inpl + ((phs + qS) + (phn_ - qN));
+        inpl = pfma(inpl, T(0.125), pc * T(0.25));
         // z direction: this plane's contribution to the planes above (up) and below (down)
-        const V uzc = lds_pair(mo + F_UZ * MF);
-        const V up(gplus(pc.x, uzc.x, nB[2].x), gplus(pc.y, uzc.y, nB[2].y));
-        const V down(gminus(pc.x, uzc.x, nB[2].x), gminus(pc.y, uzc.y, nB[2].y));
+        const V qZ = qterm(pc, lds_pair(mo + F_UZ * MF), nB[2]);
+        const V up = pc + qZ, down = pc - qZ;
         if (fin) {
           // a7: phi'(j) = inpl(j) + up(j-1)/8 + down(j+1)/8       (eqs. 23-24)
           phin = pfma(c_upa + down, T(0.125), c_inpl);
@@ -394,13 +392,16 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
         o[10] = phin;
         const long long zo = (long long)j * L.plane;
 #pragma unroll
-        for (int m = 0; m < (TWO ? 11 : 10); ++m) {
-          T *base = P.out.f[m] + zo;
-          *reinterpret_cast<V *>(base + o00) = o[m];
-          if (gxg != gx_) *reinterpret_cast<V *>(base + o10) = o[m];
-          if (gyg != gy_) {
-            *reinterpret_cast<V *>(base + o01) = o[m];
-            if (gxg != gx_) *reinterpret_cast<V *>(base + o11) = o[m];
+        for (int m = 0; m < (TWO ? 11 : 10); ++m) *reinterpret_cast<V *>(P.out.f[m] + zo + o00) = o[m];
+        if (gxg != gx_ || gyg != gy_) {          // periodic ghost images (edge tiles only)
+#pragma unroll
+          for (int m = 0; m < (TWO ? 11 : 10); ++m) {
+            T *base = P.out.f[m] + zo;
+            if (gxg != gx_) *reinterpret_cast<V *>(base + o10) = o[m];
+            if (gyg != gy_) {
+              *reinterpret_cast<V *>(base + o01) = o[m];
+              if (gxg != gx_) *reinterpret_cast<V *>(base + o11) = o[m];
+            }
           }
         }
       }
