@@ -97,7 +97,13 @@ struct TileCfg {
   static constexpr size_t OFF_ZC = OFF_NRM + (TWO ? NR * 3 * PLANE : 0);   // S_z n_x, S_z n_y, d_z n_z
   static constexpr size_t OFF_AP = OFF_ZC + (TWO ? 3 * PLANE : 0);         // y-push, upward  [9]
   static constexpr size_t OFF_AM = OFF_AP + NYP * YP_FIELD;                // y-push, downward [9]
-  static constexpr size_t OFF_BAR = OFF_AM + NYP * YP_FIELD;
+  // x exchange: per (group, row) the a+ of each pair's SECOND node (slot lx+1; slot 0 = halo column
+  // x0-1) and the a- of each pair's FIRST node (slot lx; slot LX = halo column x0+TX)
+  static constexpr int XES = LX + 1;
+  static constexpr size_t XE_BYTES = al((size_t)8 * RY * XES * sizeof(T));
+  static constexpr size_t OFF_XEP = OFF_AM + NYP * YP_FIELD;
+  static constexpr size_t OFF_XEM = OFF_XEP + XE_BYTES;
+  static constexpr size_t OFF_BAR = OFF_XEM + XE_BYTES;
   static constexpr size_t SMEM_BYTES = OFF_BAR + 64;
 };
 
@@ -171,6 +177,9 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   T *s_zc = reinterpret_cast<T *>(smem + C::OFF_ZC);
   T *s_ap = reinterpret_cast<T *>(smem + C::OFF_AP);
   T *s_am = reinterpret_cast<T *>(smem + C::OFF_AM);
+  T *s_xep = reinterpret_cast<T *>(smem + C::OFF_XEP);
+  T *s_xem = reinterpret_cast<T *>(smem + C::OFF_XEM);
+  constexpr int XES = C::XES;
 
   const Layout &L = P.L;
   const int t = threadIdx.x;
@@ -242,6 +251,39 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   const int gyg = gy_ < GY ? gy_ + L.ny : (gy_ >= L.ny - GY ? gy_ - L.ny : gy_);
   const long long o00 = L.idx(gx_, gy_, 0), o10 = L.idx(gxg, gy_, 0), o01 = L.idx(gx_, gyg, 0), o11 = L.idx(gxg, gyg, 0);
 
+  // x-pass terms of the two halo columns x0-1 (its a+) and x0+TX (its a-) of every region row of
+  // the plane held in moment slot `slot`; done by the A1 aux threads one segment ahead.
+  auto halo_cols = [&](int slot) {
+    const int e = ia - 2 * LX;
+    if (e >= 0 && e < 2 * RY) {
+      const int rr = e >> 1, side = e & 1;
+      const T *p = mom_at(slot) + rr * RX + (side ? HL + TX : HL - 1);
+      T m[10], K[NK];
+#pragma unroll
+      for (int f = 0; f < 10; ++f) m[f] = p[f * MF];
+      hermite_coeffs<ORDER, T>(m[0], m[1], m[2], m[3], m[4], m[5], m[6], m[7], m[8], m[9], P.omc, K);
+      T gp[8], gm[8], g0;
+      push3<3, T, T>(K[K000], K[K100], K[K200], gp[0], gm[0], g0);
+      push3<3, T, T>(K[K010], K[K110], K[K210], gp[1], gm[1], g0);
+      push3<2, T, T>(K[K020], K[K120], K[K120], gp[2], gm[2], g0);
+      push3<3, T, T>(K[K001], K[K101], K[K201], gp[3], gm[3], g0);
+      push3<2, T, T>(K[K011], K[K111], K[K111], gp[4], gm[4], g0);
+      push3<1, T, T>(K[K021], K[K021], K[K021], gp[5], gm[5], g0);
+      push3<2, T, T>(K[K002], K[K102], K[K102], gp[6], gm[6], g0);
+      push3<1, T, T>(K[K012], K[K012], K[K012], gp[7], gm[7], g0);
+#pragma unroll
+      for (int g = 0; g < 8; ++g) {
+        if (side == 0) s_xep[(g * RY + rr) * XES] = gp[g];
+        else s_xem[(g * RY + rr) * XES + LX] = gm[g];
+      }
+    }
+  };
+  if (!xrow) {
+    mbar_wait(&bars[0], 0u);
+    halo_cols(0);
+  }
+  __syncthreads();
+
   int ms = 0, ps = 0, ns = 0;   // ring slots of this iteration: moments i%S, phi(k-1) i%SP, n(k) i%NR
   for (int i = 0; i < NI; ++i) {
     const int k = kb + i;
@@ -256,67 +298,26 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     // =========================== segment 1 ===========================
     if (TWO && !xrow && i < NG) {
       // A1: T = S_y S_z phi, U = d_y S_z phi, V = S_y d_z phi of plane k on the region rows
-      for (int e = ia - 2 * LX; e < RY * (RX / 2); e += 2 * LX) {
-        const int rr = e / (RX / 2), cp = 2 * (e - rr * (RX / 2));
-        const int o = (rr + 1) * RX + cp;
-        V sz[3], dz[3];
+      // one thread per column pair, marching down the rows with a 3-row window of S_z phi, d_z phi
+      const int a1 = ia - 2 * LX;
+      if (a1 < RX / 2) {
+        const int cp = 2 * a1;
+        V sz0, sz1, sz2, dz0, dz1, dz2;
+        auto zrow = [&](int prow, V &sz, V &dz) {
+          const V a = lds_pair(phm + prow * RX + cp), b = lds_pair(phc + prow * RX + cp), c = lds_pair(php + prow * RX + cp);
+          sz = pfma(b, w0, (a + c) * w1);
+          dz = (c - a) * T(0.5);
+        };
+        zrow(0, sz0, dz0);
+        zrow(1, sz1, dz1);
 #pragma unroll
-        for (int d = 0; d < 3; ++d) {
-          const V a = lds_pair(phm + o + (d - 1) * RX), b = lds_pair(phc + o + (d - 1) * RX), c = lds_pair(php + o + (d - 1) * RX);
-          sz[d] = pfma(b, w0, (a + c) * w1);
-          dz[d] = (c - a) * T(0.5);
+        for (int rr = 0; rr < RY; ++rr) {
+          zrow(rr + 2, sz2, dz2);
+          sts_pair(s_tuv + rr * RX + cp, pfma(sz1, w0, (sz0 + sz2) * w1));
+          sts_pair(s_tuv + PL + rr * RX + cp, (sz2 - sz0) * T(0.5));
+          sts_pair(s_tuv + 2 * PL + rr * RX + cp, pfma(dz1, w0, (dz0 + dz2) * w1));
+          sz0 = sz1; sz1 = sz2; dz0 = dz1; dz1 = dz2;
         }
-        sts_pair(s_tuv + rr * RX + cp, pfma(sz[1], w0, (sz[0] + sz[2]) * w1));
-        sts_pair(s_tuv + PL + rr * RX + cp, (sz[2] - sz[0]) * T(0.5));
-        sts_pair(s_tuv + 2 * PL + rr * RX + cp, pfma(dz[1], w0, (dz[0] + dz[2]) * w1));
-      }
-    }
-    if (xrow && i < NG) {
-      // A2: x-pass of region row r of plane k, then the y-push terms.  A = nodes (x-1, x), B = (x+1, x+2).
-      V KA[NK], KB[NK];
-      {
-        V mA[10], mB[10];
-        const T *p = mom_at(ms) + oM;
-#pragma unroll
-        for (int f = 0; f < 10; ++f) {
-          mA[f] = V(p[f * MF - 1], p[f * MF]);
-          mB[f] = V(p[f * MF + 1], p[f * MF + 2]);
-        }
-        hermite_coeffs<ORDER, V>(mA[0], mA[1], mA[2], mA[3], mA[4], mA[5], mA[6], mA[7], mA[8], mA[9], omc, KA);
-        hermite_coeffs<ORDER, V>(mB[0], mB[1], mB[2], mB[3], mB[4], mB[5], mB[6], mB[7], mB[8], mB[9], omc, KB);
-      }
-      V Xb[3][3];   // [b][p] of the current c
-      // c = 0: groups (b,c) = (0,0) a=0,1,2 | (1,0) a=0,1,2 | (2,0) a=0,1
-      xgroup<3, V, T>(KA, KB, K000, K100, K200, Xb[0][0], Xb[0][1], Xb[0][2]);
-      xgroup<3, V, T>(KA, KB, K010, K110, K210, Xb[1][0], Xb[1][1], Xb[1][2]);
-      xgroup<2, V, T>(KA, KB, K020, K120, 0, Xb[2][0], Xb[2][1], Xb[2][2]);
-#pragma unroll
-      for (int p = 0; p < 3; ++p) {
-        V ap, am;
-        push3<3, V, T>(Xb[0][p], Xb[1][p], Xb[2][p], ap, am, A0[p]);
-        sts_pair(s_ap + p * YPF + oY, ap);
-        sts_pair(s_am + p * YPF + oY, am);
-      }
-      // c = 1: (0,1) a=0,1,2 | (1,1) a=0,1 | (2,1) a=0
-      xgroup<3, V, T>(KA, KB, K001, K101, K201, Xb[0][0], Xb[0][1], Xb[0][2]);
-      xgroup<2, V, T>(KA, KB, K011, K111, 0, Xb[1][0], Xb[1][1], Xb[1][2]);
-      xgroup<1, V, T>(KA, KB, K021, 0, 0, Xb[2][0], Xb[2][1], Xb[2][2]);
-#pragma unroll
-      for (int p = 0; p < 3; ++p) {
-        V ap, am;
-        push3<3, V, T>(Xb[0][p], Xb[1][p], Xb[2][p], ap, am, A0[3 + p]);
-        sts_pair(s_ap + (3 + p) * YPF + oY, ap);
-        sts_pair(s_am + (3 + p) * YPF + oY, am);
-      }
-      // c = 2: (0,2) a=0,1 | (1,2) a=0
-      xgroup<2, V, T>(KA, KB, K002, K102, 0, Xb[0][0], Xb[0][1], Xb[0][2]);
-      xgroup<1, V, T>(KA, KB, K012, 0, 0, Xb[1][0], Xb[1][1], Xb[1][2]);
-#pragma unroll
-      for (int p = 0; p < 3; ++p) {
-        V ap, am;
-        push3<2, V, T>(Xb[0][p], Xb[1][p], Xb[1][p], ap, am, A0[6 + p]);
-        sts_pair(s_ap + (6 + p) * YPF + oY, ap);
-        sts_pair(s_am + (6 + p) * YPF + oY, am);
       }
     }
     if (!aux && i >= 1) {
@@ -406,10 +407,56 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
         }
       }
     }
+    if (xrow && i < NG) {
+      // A2: x-pass of region row r of plane k in push form, then the y-push terms.  Each node's K is
+      // evaluated once; a+ / a- cross to the x-neighbour thread through shared memory (same warp).
+      V Xg[8][3];   // [group][p]
+      {
+        V m[10], K[NK];
+        const T *p = mom_at(ms) + oM;
+#pragma unroll
+        for (int f = 0; f < 10; ++f) m[f] = lds_pair(p + f * MF);
+        hermite_coeffs<ORDER, V>(m[0], m[1], m[2], m[3], m[4], m[5], m[6], m[7], m[8], m[9], omc, K);
+        V gp[8], gm[8], g0[8];
+        push3<3, V, T>(K[K000], K[K100], K[K200], gp[0], gm[0], g0[0]);   // (b,c) = (0,0)
+        push3<3, V, T>(K[K010], K[K110], K[K210], gp[1], gm[1], g0[1]);   // (1,0)
+        push3<2, V, T>(K[K020], K[K120], K[K120], gp[2], gm[2], g0[2]);   // (2,0)
+        push3<3, V, T>(K[K001], K[K101], K[K201], gp[3], gm[3], g0[3]);   // (0,1)
+        push3<2, V, T>(K[K011], K[K111], K[K111], gp[4], gm[4], g0[4]);   // (1,1)
+        push3<1, V, T>(K[K021], K[K021], K[K021], gp[5], gm[5], g0[5]);   // (2,1)
+        push3<2, V, T>(K[K002], K[K102], K[K102], gp[6], gm[6], g0[6]);   // (0,2)
+        push3<1, V, T>(K[K012], K[K012], K[K012], gp[7], gm[7], g0[7]);   // (1,2)
+        T *xp = s_xep + r * XES + lx, *xm = s_xem + r * XES + lx;
+#pragma unroll
+        for (int g = 0; g < 8; ++g) { xp[g * RY * XES + 1] = gp[g].y; xm[g * RY * XES] = gm[g].x; }
+        __syncwarp();
+#pragma unroll
+        for (int g = 0; g < 8; ++g) {
+          const V up(xp[g * RY * XES], gp[g].x), dn(gm[g].y, xm[g * RY * XES + 1]);
+          pull3<V, T>(up, dn, g0[g], Xg[g][0], Xg[g][1], Xg[g][2]);
+        }
+      }
+      // y-push per (c, p): groups of c = 0: b = 0,1,2 -> g 0,1,2; c = 1: g 3,4,5; c = 2: b = 0,1 -> g 6,7
+#pragma unroll
+      for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int p = 0; p < 3; ++p) {
+          V ap, am;
+          if (c < 2) push3<3, V, T>(Xg[3 * c][p], Xg[3 * c + 1][p], Xg[3 * c + 2][p], ap, am, A0[3 * c + p]);
+          else push3<2, V, T>(Xg[6][p], Xg[7][p], Xg[7][p], ap, am, A0[6 + p]);
+          sts_pair(s_ap + (3 * c + p) * YPF + oY, ap);
+          sts_pair(s_am + (3 * c + p) * YPF + oY, am);
+        }
+    }
     __syncthreads();
     if (t == 0 && i + 2 < NG) issue(i + 2);
 
     // =========================== segment 2 ===========================
+    if (!xrow && i + 1 < NG) {
+      const int sl = ms == S - 1 ? 0 : ms + 1;
+      mbar_wait(&bars[sl], (uint32_t)(((i + 1) / S) & 1));
+      halo_cols(sl);
+    }
     if (i < NG) {
       if (!aux) {
         // B2: finish the y-pass (a+ from the row below, a- from the row above, own a0) and z-push.
