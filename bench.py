@@ -36,8 +36,8 @@ CONFIGS = {
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=30)
-    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--config", default=os.environ.get("TSLB_BENCH_CONFIG", "c5"))
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--precision", default="f32")
@@ -200,6 +200,7 @@ def main():
     import torch
     import torch.distributed as dist
     from paper_2403_15773_b200 import build, inputs, tslb
+    from paper_2403_15773_b200 import dist as tdist
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -231,8 +232,7 @@ def main():
 
     def barrier():
         torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
+        tdist.barrier()
         torch.cuda.synchronize()
 
     # ---- device-resident timing: W warm-up steps, then exactly K steps between CUDA events on the
@@ -256,11 +256,8 @@ def main():
     m = sim.get_moments(device=True, want=("rho", "phi"))
     finite = bool(torch.isfinite(m["rho"]).all().item() and torch.isfinite(m["phi"]).all().item())
     del m
-    tmax = torch.tensor([ms], device=dev)
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms_max = float(tmax.item())
-    glups = world * nodes * args.steps / (ms_max * 1e-3) / 1e9
+    ms_max = tdist.max_over_ranks(ms, dev)
+    glups = tdist.job_throughput(nodes * args.steps, ms * 1e-3, dev) / 1e9
 
     # ---- end to end through the C-ABI with HOST buffers: H2D of the inputs, K steps, D2H of the state
     e2e = None
@@ -287,10 +284,7 @@ def main():
         torch.cuda.synchronize()
         w1 = time.perf_counter()
         esz = 4 if prec == tslb.F32 else 8
-        tw = torch.tensor([w1 - w0], device=dev)
-        if world > 1:
-            dist.all_reduce(tw, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * nodes * args.steps / float(tw.item()) / 1e9, "unit": "GLUPS",
+        e2e = {"value": tdist.job_throughput(nodes * args.steps, w1 - w0, dev) / 1e9, "unit": "GLUPS",
                "h2d_bytes_per_step": 5 * nodes * esz / args.steps, "d2h_bytes_per_step": 11 * nodes * esz / args.steps,
                "what": "tslb_init_fields(host) + tslb_step(K) + tslb_get_moments(host), pinned host buffers, "
                        "wall clock; bytes are the job's total divided by K"}
@@ -325,7 +319,7 @@ def main():
 
     cpu = None
     if not args.no_cpu:
-        g, threads, sample, _ = oracle_sample(args.config, 2)
+        g, threads, sample, _ = oracle_sample(args.config, 6)
         cpu = {"value": g, "unit": "GLUPS", "cores": threads, "kind": "oracle", "sample": sample}
 
     out = {"metric": "GLUPS (fused flow+phase-field step)", "value": glups, "unit": "GLUPS", "n_gpus": world,

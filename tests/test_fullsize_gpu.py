@@ -1,0 +1,101 @@
+"""Parity at BASELINE.json's FULL size (configs[4], 512x512x1536 fp32 jet) in the launch
+configuration bench.py times, on sampled outputs the oracle can compute one by one.
+
+After s steps the value at a node depends only on the initial fields within 2s+2 cells of it, so
+a (w^3) window cut out of the full-size initial state, stepped by the oracle as a small periodic
+box, reproduces the full-size result on the window's interior (margin 2s+2).  The two z boundary
+planes are covered by full-x-y slabs stepped by the oracle with the jet boundary conditions.
+Error norm: SURVEY N2 over the union of the sampled nodes; fp32 gate 1e-5."""
+import numpy as np
+import pytest
+
+from oracle import ref
+from paper_2403_15773_b200 import inputs, tslb
+
+pytestmark = pytest.mark.gpu
+
+STEPS = 2
+MARGIN = 2 * STEPS + 2
+
+
+def _window(t, x0, y0, z0, w):
+    import torch
+    nz, ny, nx = t.shape
+    ix = (torch.arange(x0, x0 + w, device=t.device) % nx)
+    iy = (torch.arange(y0, y0 + w, device=t.device) % ny)
+    return t[z0:z0 + w][:, iy][:, :, ix].double().cpu().numpy()
+
+
+def test_c5_full_size_sampled_against_oracle():
+    import torch
+    import bench
+    if torch.cuda.get_device_properties(0).total_memory < 90e9:
+        pytest.skip("needs ~75 GB of device memory")
+    nx, ny, nz, D, _ = bench.CONFIGS["c5"]
+    prm = inputs.jet_params(nx, ny, nz, D, We=2000.0)
+    dev = torch.device("cuda", 0)
+    st = bench.developed_jet_device(torch, nx, ny, nz, D, prm["jet_velocity"], torch.float32, dev)
+    # seeded transverse velocity noise so that every moment is non-trivial
+    g = torch.Generator(device=dev).manual_seed(4321)
+    for k in ("ux", "uy"):
+        st[k] = (torch.rand((nz, ny, nx), generator=g, device=dev, dtype=torch.float32) - 0.5) * 0.004
+    kw = {k: v for k, v in prm.items() if k not in ("nx", "ny", "nz", "omega")}
+    sim = tslb.Tslb(nx, ny, nz, prm["omega"], precision=tslb.F32, **kw)   # same selection as bench.py
+    assert "tiled" in sim.kernel_name
+    sim.init_fields(st["rho"], st["ux"], st["uy"], st["uz"], st["phi"])
+    sim.step(STEPS)
+    out = sim.get_moments(device=True)
+    names = ("rho", "ux", "uy", "uz", "phi")
+    okw = dict(two_component=True, sigma=prm["sigma"], interface_width=prm["interface_width"])
+    num = dict(rho=0.0, u=0.0, pineq=0.0, phi=0.0)
+    den = dict(rho=0.0, u=0.0, pineq=0.0, phi=0.0)
+
+    def accumulate(gpu, refm, sl):
+        for k in ("rho", "phi"):
+            num[k] = max(num[k], np.abs(gpu[k][sl] - refm[k][sl]).max()); den[k] = max(den[k], np.abs(refm[k][sl]).max())
+        for k in ("ux", "uy", "uz"):
+            num["u"] = max(num["u"], np.abs(gpu[k][sl] - refm[k][sl]).max()); den["u"] = max(den["u"], np.abs(refm[k][sl]).max())
+        num["pineq"] = max(num["pineq"], np.abs(gpu["pineq"][(slice(None),) + sl] - refm["pineq"][(slice(None),) + sl]).max())
+        den["pineq"] = max(den["pineq"], np.abs(refm["pineq"][(slice(None),) + sl]).max())
+
+    # interior windows: jet core, tile / chunk / periodic edges, core end, downstream cone
+    w = 28
+    windows = [(242, 242, 60), (498, 500, 700), (250, 3, 114), (20, 250, 370), (262, 236, 498),
+               (236, 262, 1010), (240, 250, 1266)]
+    for (x0, y0, z0) in windows:
+        ini = {k: _window(st[k], x0, y0, z0, w) for k in names}
+        o = ref.Oracle(w, w, w, prm["omega"], **okw)
+        o.init_fields(ini["rho"], ini["ux"], ini["uy"], ini["uz"], ini["phi"])
+        o.step(STEPS)
+        r = o.get_moments()
+        o.close()
+        gpu = {k: _window(out[k], x0, y0, z0, w) for k in names}
+        gpu["pineq"] = np.stack([_window(out["pineq"][c], x0, y0, z0, w) for c in range(6)])
+        m = MARGIN
+        accumulate(gpu, r, (slice(m, w - m), slice(m, w - m), slice(m, w - m)))
+
+    # boundary slabs (full x-y): inflow at z = 0 and outflow at z = nz-1
+    sz = 14
+    jet = dict(bc_zlo=ref.BC_JET_INFLOW, bc_zhi=ref.BC_OUTFLOW, jet_diameter=prm["jet_diameter"],
+               jet_velocity=prm["jet_velocity"], jet_perturbation=prm["jet_perturbation"], seed=prm["seed"])
+    for zlo, keep in ((0, slice(0, sz - MARGIN)), (nz - sz, slice(MARGIN, sz))):
+        ini = {k: st[k][zlo:zlo + sz].double().cpu().numpy() for k in names}
+        o = ref.Oracle(nx, ny, sz, prm["omega"], **okw, **jet)
+        o.init_fields(ini["rho"], ini["ux"], ini["uy"], ini["uz"], ini["phi"])
+        if zlo != 0:
+            # the slab's own z = 0 plane is not the real inflow plane: it is excluded by `keep`
+            pass
+        o.step(STEPS)
+        r = o.get_moments()
+        o.close()
+        gpu = {k: out[k][zlo:zlo + sz].double().cpu().numpy() for k in names}
+        gpu["pineq"] = np.stack([out["pineq"][c][zlo:zlo + sz].double().cpu().numpy() for c in range(6)])
+        accumulate(gpu, r, (keep, slice(None), slice(None)))
+
+    err = {k: num[k] / max(den[k], 1e-300) for k in num}
+    print("full-size sampled parity (fp32, %d steps):" % STEPS, err, "scales", den)
+    assert den["u"] > 0.04 and den["phi"] > 0.99 and den["pineq"] > 1e-6
+    for k, v in err.items():
+        assert v <= 1e-5, (k, v)
+    assert bool(torch.isfinite(out["rho"]).all()) and bool(torch.isfinite(out["phi"]).all())
+    sim.close()
