@@ -114,11 +114,13 @@ struct TiledMaps {
   int zc;            // planes per z chunk
 };
 
-template <typename T> __device__ __forceinline__ Pair<T> prcp(Pair<T> a);
-template <> __device__ __forceinline__ F2 prcp<float>(F2 a) { return F2(__frcp_rn(a.x), __frcp_rn(a.y)); }
-template <> __device__ __forceinline__ D2 prcp<double>(D2 a) { return D2(1.0 / a.x, 1.0 / a.y); }
-__device__ __forceinline__ float rcp1(float s) { return __frcp_rn(s); }
+// Reciprocal and square root.  fp32: the branch-free MUFU approximations (<= 2 ulp, far inside the
+// 1e-5 parity gate; rho' ~ 1 and |G| + eps >= 1e-12 are normal numbers); fp64: IEEE.
+__device__ __forceinline__ float rcp1(float s) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(s)); return r; }
 __device__ __forceinline__ double rcp1(double s) { return 1.0 / s; }
+__device__ __forceinline__ float sqrt1(float s) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(s)); return r; }
+__device__ __forceinline__ double sqrt1(double s) { return sqrt(s); }
+template <typename T> __device__ __forceinline__ Pair<T> prcp(Pair<T> a) { return Pair<T>(rcp1(a.x), rcp1(a.y)); }
 
 // The 1-D three-point operator of the tensor-product basis in PUSH form.  A source
 // node holding the un-normalised Hermite coefficients g_0, g_1, g_2 (index along this axis) sends
@@ -239,7 +241,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   V A0[9];                  // this row's own y-push term a0 per (c,p), carried across the barrier
   V nA[3], nB[3];           // own n of planes k-2 and k-1
   V gA(T(0)), gB(T(0));     // own |G| of planes k-2 and k-1
-  V c_inpl(T(0)), c_upa(T(0)), c_upb(T(0));
+  V c_inpl(T(0)), c_upa(T(0)), c_upb(T(0)), c_rinv(T(1));
 #pragma unroll
   for (int m = 0; m < 10; ++m) { accA[m] = V(T(0)); accB[m] = V(T(0)); fl[m] = V(T(0)); }
 #pragma unroll
@@ -377,8 +379,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
           kap.x += w1 * eN.x + w0 * eO.x + w1 * eO.y;                        // S_x S_y c
           kap.y += w1 * eO.x + w0 * eO.y + w1 * eN.y;
           // a6: F = sigma kappa G, kappa = -div n, G = n (|G| + eps); u' = u_b + F / rho'
-          const V rinv = prcp<T>(fl[0] + V(T(1)));
-          const V sc = (kap * (gA + V(T(1e-12)))) * rinv * (-P.sigma);
+          const V sc = (kap * (gA + V(T(1e-12)))) * c_rinv * (-P.sigma);
           ukx = nA[0] * sc; uky = nA[1] * sc; ukz = nA[2] * sc;
         }
         c_upa = c_upb; c_upb = up; c_inpl = inpl;
@@ -496,6 +497,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
         }
         // a4: plane k-1 is complete: u_b = m'/rho', Pi^neq' = Pi' - rho' u_b u_b (Hermite form)
         const V inv = prcp<T>(outm[0] + V(T(1)));
+        c_rinv = inv;
         fl[0] = outm[0];
         fl[1] = outm[1] * inv; fl[2] = outm[2] * inv; fl[3] = outm[3] * inv;
         fl[4] = outm[4] - outm[1] * fl[1];
@@ -516,7 +518,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
           const V gy(w1 * (ul + uc.y) + w0 * uc.x, w1 * (uc.x + ur) + w0 * uc.y);
           const V gz(w1 * (vl + vc.y) + w0 * vc.x, w1 * (vc.x + vr) + w0 * vc.y);
           const V s2 = pfma(gz, gz, pfma(gy, gy, gx * gx));
-          mag = V(tsqrt<T>(s2.x), tsqrt<T>(s2.y));                                  // |G|
+          mag = V(sqrt1(s2.x), sqrt1(s2.y));                                  // |G|
           const V inv(rcp1(mag.x + T(1e-12)), rcp1(mag.y + T(1e-12)));             // reading A7
           nn[0] = gx * inv; nn[1] = gy * inv; nn[2] = gz * inv;
           sts_pair(nk + o, nn[0]); sts_pair(nk + PL + o, nn[1]); sts_pair(nk + 2 * PL + o, nn[2]);
