@@ -97,13 +97,12 @@ struct TileCfg {
   static constexpr size_t OFF_ZC = OFF_NRM + (TWO ? NR * 3 * PLANE : 0);   // S_z n_x, S_z n_y, d_z n_z
   static constexpr size_t OFF_AP = OFF_ZC + (TWO ? 3 * PLANE : 0);         // y-push, upward  [9]
   static constexpr size_t OFF_AM = OFF_AP + NYP * YP_FIELD;                // y-push, downward [9]
-  // x exchange: per (group, row) the a+ of each pair's SECOND node (slot lx+1; slot 0 = halo column
-  // x0-1) and the a- of each pair's FIRST node (slot lx; slot LX = halo column x0+TX)
-  static constexpr int XES = LX + 1;
-  static constexpr size_t XE_BYTES = al((size_t)8 * RY * XES * sizeof(T));
-  static constexpr size_t OFF_XEP = OFF_AM + NYP * YP_FIELD;
-  static constexpr size_t OFF_XEM = OFF_XEP + XE_BYTES;
-  static constexpr size_t OFF_BAR = OFF_XEM + XE_BYTES;
+  // x exchange.  Inside a warp the a+ of each pair's second node / a- of its first node cross
+  // through the warp's OWN first row of the y-push fields 0..7 (dead at that time).  Only the terms
+  // of the two halo columns x0-1 (a+) and x0+TX (a-) need storage of their own: [2][8][RY].
+  static constexpr size_t XH_BYTES = al((size_t)2 * 8 * RY * sizeof(T));
+  static constexpr size_t OFF_XH = OFF_AM + NYP * YP_FIELD;
+  static constexpr size_t OFF_BAR = OFF_XH + XH_BYTES;
   static constexpr size_t SMEM_BYTES = OFF_BAR + 64;
 };
 
@@ -179,9 +178,8 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   T *s_zc = reinterpret_cast<T *>(smem + C::OFF_ZC);
   T *s_ap = reinterpret_cast<T *>(smem + C::OFF_AP);
   T *s_am = reinterpret_cast<T *>(smem + C::OFF_AM);
-  T *s_xep = reinterpret_cast<T *>(smem + C::OFF_XEP);
-  T *s_xem = reinterpret_cast<T *>(smem + C::OFF_XEM);
-  constexpr int XES = C::XES;
+  T *s_xhl = reinterpret_cast<T *>(smem + C::OFF_XH);      // a+ of column x0-1   [8][RY]
+  T *s_xhr = s_xhl + 8 * RY;                                // a- of column x0+TX  [8][RY]
 
   const Layout &L = P.L;
   const int t = threadIdx.x;
@@ -194,6 +192,9 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   const int oM = r * RX + c0;                             // offset of the pair in a region plane
   const int oY = r * TX + 2 * lx;                         // offset of the pair in a y-push field
   const int ia = (tr - TY) * LX + lx;                     // aux thread index
+  // x-exchange word of this lane: word (t & 31) of the y-push row owned by lane 0 of the warp
+  const int trf = (t & ~31) / LX;
+  const int oX = (trf < TY ? trf + 1 : (trf == TY ? 0 : RY - 1)) * TX + (t & 31);
   const int x0 = (blockIdx.x % M.ntx) * TX;
   const int y0 = (blockIdx.x / M.ntx) * TY;
   const int z0 = blockIdx.y * M.zc;
@@ -275,8 +276,8 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
       push3<1, T, T>(K[K012], K[K012], K[K012], gp[7], gm[7], g0);
 #pragma unroll
       for (int g = 0; g < 8; ++g) {
-        if (side == 0) s_xep[(g * RY + rr) * XES] = gp[g];
-        else s_xem[(g * RY + rr) * XES + LX] = gm[g];
+        if (side == 0) s_xhl[g * RY + rr] = gp[g];
+        else s_xhr[g * RY + rr] = gm[g];
       }
     }
   };
@@ -427,15 +428,20 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
         push3<1, V, T>(K[K021], K[K021], K[K021], gp[5], gm[5], g0[5]);   // (2,1)
         push3<2, V, T>(K[K002], K[K102], K[K102], gp[6], gm[6], g0[6]);   // (0,2)
         push3<1, V, T>(K[K012], K[K012], K[K012], gp[7], gm[7], g0[7]);   // (1,2)
-        T *xp = s_xep + r * XES + lx, *xm = s_xem + r * XES + lx;
+        // lane l of the warp parks gp.y / gm.x at word l of the warp's first y-push row
+        T *xp = s_ap + oX, *xm = s_am + oX;
 #pragma unroll
-        for (int g = 0; g < 8; ++g) { xp[g * RY * XES + 1] = gp[g].y; xm[g * RY * XES] = gm[g].x; }
+        for (int g = 0; g < 8; ++g) { xp[g * YPF] = gp[g].y; xm[g * YPF] = gm[g].x; }
         __syncwarp();
+        // left / right neighbour's word, or the halo column's term for the lanes at the tile edge
+        const T *pl = lx == 0 ? s_xhl + r : xp - 1, *pr = lx == LX - 1 ? s_xhr + r : xm + 1;
+        const int sl = lx == 0 ? RY : YPF, sr = lx == LX - 1 ? RY : YPF;
 #pragma unroll
         for (int g = 0; g < 8; ++g) {
-          const V up(xp[g * RY * XES], gp[g].x), dn(gm[g].y, xm[g * RY * XES + 1]);
+          const V up(pl[g * sl], gp[g].x), dn(gm[g].y, pr[g * sr]);
           pull3<V, T>(up, dn, g0[g], Xg[g][0], Xg[g][1], Xg[g][2]);
         }
+        __syncwarp();
       }
       // y-push per (c, p): groups of c = 0: b = 0,1,2 -> g 0,1,2; c = 1: g 3,4,5; c = 2: b = 0,1 -> g 6,7
 #pragma unroll
