@@ -61,6 +61,10 @@ __device__ __forceinline__ D2 pfma(D2 a, D2 b, D2 c) { return D2(fma(a.x, b.x, c
 __device__ __forceinline__ D2 pfma(D2 a, double s, D2 c) { return D2(fma(a.x, s, c.x), fma(a.y, s, c.y)); }
 __device__ __forceinline__ D2 operator*(D2 a, double s) { return D2(a.x * s, a.y * s); }
 
+__device__ __forceinline__ F2 pneg(F2 a) { return F2(-a.x, -a.y); }
+__device__ __forceinline__ D2 pneg(D2 a) { return D2(-a.x, -a.y); }
+__device__ __forceinline__ float pneg(float a) { return -a; }
+__device__ __forceinline__ double pneg(double a) { return -a; }
 // scalar overloads so the same templates serve the one-node-per-thread kernels
 __device__ __forceinline__ float pfma(float a, float b, float c) { return fmaf(a, b, c); }
 __device__ __forceinline__ double pfma(double a, double b, double c) { return fma(a, b, c); }

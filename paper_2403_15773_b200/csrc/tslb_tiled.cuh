@@ -134,8 +134,7 @@ __device__ __forceinline__ void push3(V g0, V g1, V g2, V &ap, V &am, V &a0) {
   if (NA == 3) h = pfma(g2, T(0.5), h);
   ap = h; am = h;
   if (NA >= 2) { ap = pfma(g1, T(0.5), h); am = pfma(g1, T(-0.5), h); }
-  a0 = g0 * T(2.0 / 3.0);
-  if (NA == 3) a0 = a0 - g2;
+  a0 = NA == 3 ? pfma(g0, T(2.0 / 3.0), pneg(g2)) : g0 * T(2.0 / 3.0);
 }
 // destination side: from up = a+(-1), dn = a-(+1), a0 -> W0, W1, W2
 template <typename V, typename T>
@@ -143,20 +142,15 @@ __device__ __forceinline__ void pull3(V up, V dn, V a0, V &W0, V &W1, V &W2) {
   const V s = up + dn;
   W0 = s + a0;
   W1 = up - dn;
-  W2 = pfma(s, T(2.0 / 3.0), a0 * T(-1.0 / 3.0));
+  W2 = pfma(W0, T(2.0 / 3.0), pneg(a0));     // = 2/3 s - a0/3
 }
-
-// x-pass of one (b,c) group for the node pair (x, x+1) from the coefficients on the shifted pairs
-// A = (x-1, x) and B = (x+1, x+2): a+ is needed at A, a- at B and a0 at (A.y, B.x).
-template <int NA, typename V, typename T>
-__device__ __forceinline__ void xgroup(const V *KA, const V *KB, int i0, int i1, int i2, V &X0, V &X1, V &X2) {
-  V hA = KA[i0] * T(1.0 / 6.0), hB = KB[i0] * T(1.0 / 6.0);
-  if (NA == 3) { hA = pfma(KA[i2], T(0.5), hA); hB = pfma(KB[i2], T(0.5), hB); }
-  V ap = hA, am = hB;
-  if (NA >= 2) { ap = pfma(KA[i1], T(0.5), hA); am = pfma(KB[i1], T(-0.5), hB); }
-  V a0(T(2.0 / 3.0) * KA[i0].y, T(2.0 / 3.0) * KB[i0].x);
-  if (NA == 3) { a0.x -= KA[i2].y; a0.y -= KB[i2].x; }
-  pull3<V, T>(ap, am, a0, X0, X1, X2);
+// the same with up = (l, upy) and dn = (dnx, r) given as scalars from two different register pairs
+template <typename V, typename T>
+__device__ __forceinline__ void pull3s(T l, T upy, T dnx, T r, V a0, V &W0, V &W1, V &W2) {
+  const V s(l + dnx, upy + r);
+  W0 = s + a0;
+  W1 = V(l - dnx, upy - r);
+  W2 = pfma(W0, T(2.0 / 3.0), pneg(a0));
 }
 
 // ------------------------------------------------------------------ the kernel
@@ -438,8 +432,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
         const int sl = lx == 0 ? RY : YPF, sr = lx == LX - 1 ? RY : YPF;
 #pragma unroll
         for (int g = 0; g < 8; ++g) {
-          const V up(pl[g * sl], gp[g].x), dn(gm[g].y, pr[g * sr]);
-          pull3<V, T>(up, dn, g0[g], Xg[g][0], Xg[g][1], Xg[g][2]);
+          pull3s<V, T>(pl[g * sl], gp[g].x, gm[g].y, pr[g * sr], g0[g], Xg[g][0], Xg[g][1], Xg[g][2]);
         }
         __syncwarp();
       }
