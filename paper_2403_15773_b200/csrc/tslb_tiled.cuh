@@ -330,12 +330,13 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
         const V gamv(P.gamma);
         auto qterm = [&](V p, V u, V n) { return p * pfma(pfma(p, V(T(0)) - gamv, gamv), n, u * T(4)); };
         const V pc = lds_pair(ph);
-        // x direction: g+ at columns (c0-1, c0), g- at columns (c0+1, c0+2)
+        // x direction: node x gets g+(c0-1) + g-(c0+1), node x+1 gets g+(c0) + g-(c0+2)
         const V uxc = lds_pair(mo + F_UX * MF);
-        const V pA(ph[-1], pc.x), pB(pc.y, ph[2]);
-        const V qA = qterm(pA, V(mo[F_UX * MF - 1], uxc.x), V(nr[-1], nB[0].x));
-        const V qB = qterm(pB, V(uxc.y, mo[F_UX * MF + 2]), V(nB[0].y, nr[2]));
-        V inpl = (pA + qA) + (pB - qB);
+        // (q on the own columns and on the two outer columns c0-1, c0+2; mixed only at the end)
+        const V pn(ph[-1], ph[2]);
+        const V qO = qterm(pc, uxc, nB[0]);
+        const V qX = qterm(pn, V(mo[F_UX * MF - 1], mo[F_UX * MF + 2]), V(nr[-1], nr[2]));
+        V inpl((pn.x + qX.x) + (pc.y - qO.y), (pc.x + qO.x) + (pn.y - qX.y));
         // y direction: rows r-1 (south, c_i = +e_y) and r+1 (north)
         const V phs = lds_pair(ph - RX), phn_ = lds_pair(ph + RX);
         const V qS = qterm(phs, lds_pair(mo + F_UY * MF - RX), lds_pair(nr + PL - RX));
