@@ -632,12 +632,20 @@ inline bool tiled_plan_create(TiledPlan &pl, int precision, const Layout &L, voi
     pl.maps[b].ntx = L.nx / pl.tx;
     pl.maps[b].nty = L.ny / pl.ty;
   }
-  // z chunking: enough CTAs to fill the machine several times, chunks long enough to amortise the
-  // 3-plane pipeline prologue
+  // z chunking: every chunk pays a 3-plane pipeline prologue, and the grid runs in waves of
+  // (CTAs per SM) x (SM count): pick the chunk length that minimises waves x (zc + 3).
   const long long tiles = (long long)(L.nx / pl.tx) * (L.ny / pl.ty);
-  int zc = 128;
-  while (zc > 8 && tiles * ((L.nz + zc - 1) / zc) < 4 * 148) zc /= 2;
-  if (zc > L.nz) zc = L.nz;
+  int nsm = 148;
+  cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, device);
+  const long long slots = (long long)nsm * (precision == TSLB_F32 ? 2 : 1);
+  int zc = L.nz;
+  long long best = -1;
+  for (int cand = 8; cand <= 128; cand *= 2) {
+    const int c = cand < L.nz ? cand : L.nz;
+    const long long ctas = tiles * ((L.nz + c - 1) / c);
+    const long long cost = ((ctas + slots - 1) / slots) * (c + 3);
+    if (best < 0 || cost < best) { best = cost; zc = c; }
+  }
   if (const char *env = getenv("TSLB_ZCHUNK")) { int v = atoi(env); if (v > 0) zc = v; }
   pl.zc = zc;
   pl.maps[0].zc = pl.maps[1].zc = zc;
