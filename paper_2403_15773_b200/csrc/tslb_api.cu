@@ -12,6 +12,9 @@
 #include "../../include/tslb.h"
 #include "tslb_generic.cuh"
 #include "tslb_tiled.cuh"
+#include "tslb_tiled_ws.cuh"
+
+#include <type_traits>
 
 using namespace tslb;
 
@@ -90,6 +93,7 @@ struct tslb_ctx {
   long long launches = 0;
   void *stage = nullptr;       // one dense field, for host <-> device import/export
   TiledPlan tiled;             // TMA descriptors etc.
+  bool use_ws = false;         // warp-specialised variant of the tiled kernel (fp32, two-component)
   std::string err;
   std::string kname;
 
@@ -165,7 +169,13 @@ int step_typed(tslb_ctx *c, int nsteps) {
     StepParams<T> P = make_step_params<T>(c, c->cur, c->cur ^ 1);
     int rc;
     if (c->v.kernel == TSLB_KERNEL_TILED) {
-      cudaError_t e = launch_tiled<T>(c->tiled, P, c->cur, c->p.hermite_order, c->p.two_component != 0, c->stream);
+      cudaError_t e;
+      if constexpr (std::is_same<T, float>::value) {
+        e = c->use_ws ? launch_tiled_ws<TSLB_F32_TX, TSLB_TY>(c->tiled, P, c->cur, c->p.hermite_order, c->stream)
+                      : launch_tiled<T>(c->tiled, P, c->cur, c->p.hermite_order, c->p.two_component != 0, c->stream);
+      } else {
+        e = launch_tiled<T>(c->tiled, P, c->cur, c->p.hermite_order, c->p.two_component != 0, c->stream);
+      }
       c->launches += c->v.zper ? 1 : 2;   // + the boundary-plane kernel with inflow/outflow
       rc = (e == cudaSuccess) ? TSLB_OK : c->cuda_fail(e, "launch_tiled");
     } else {
@@ -307,7 +317,11 @@ int tslb_create(const tslb_params *p, tslb_ctx **out) {
       delete c;
       return TSLB_ECUDA;
     }
-    c->kname = c->tiled.name;
+    if (p->precision == TSLB_F32 && p->two_component && TSLB_F32_TX == 32 && TSLB_TY == 8) {
+      const char *env = getenv("TSLB_WS");
+      c->use_ws = env ? atoi(env) != 0 : false;
+    }
+    c->kname = c->use_ws ? "tiled-ws" + c->tiled.name.substr(5) : c->tiled.name;
   } else {
     c->kname = "generic";
   }
