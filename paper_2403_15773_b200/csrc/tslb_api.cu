@@ -170,8 +170,8 @@ int step_typed(tslb_ctx *c, int nsteps) {
     int rc;
     if (c->v.kernel == TSLB_KERNEL_TILED) {
       cudaError_t e;
-      if constexpr (std::is_same<T, float>::value) {
-        e = c->use_ws ? launch_tiled_ws<TSLB_F32_TX, TSLB_TY>(c->tiled, P, c->cur, c->p.hermite_order, c->stream)
+      if constexpr (std::is_same<T, float>::value && TSLB_F32_TX == 32 && TSLB_TY == 8) {
+        e = c->use_ws ? launch_tiled_ws<32, 8>(c->tiled, P, c->cur, c->p.hermite_order, c->stream)
                       : launch_tiled<T>(c->tiled, P, c->cur, c->p.hermite_order, c->p.two_component != 0, c->stream);
       } else {
         e = launch_tiled<T>(c->tiled, P, c->cur, c->p.hermite_order, c->p.two_component != 0, c->stream);
