@@ -8,8 +8,8 @@
 //
 // The 27-neighbour pull of PAPER.md:98 eq. 6 / Fig. 1 is evaluated in the tensor-product Hermite
 // basis (tslb_math.cuh) as three 1-D three-point passes:
-//   x-pass  (segment 1)  K_abc (17 per node, recomputed for the pair's two x-neighbours)
-//                        -> X^p_bc (24 per node, registers);
+//   x-pass  (segment 1)  K_abc (17 per node, evaluated once) in push form: a+ / a- cross to the
+//                        neighbouring lane inside the warp -> X^p_bc (24 per node, registers);
 //   y-push  (seg. 1->2)  every row forms, per (p,c), the combination a+ it sends to the row above,
 //                        a- it sends to the row below and a0 it keeps: only 9+9 values per node
 //                        cross shared memory (not 24 x 3 rows) -> Y^pq_c (18, registers);
