@@ -185,6 +185,9 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   const int c0 = HL + 2 * lx;                             // staged column of the pair's first node
   const int oM = r * RX + c0;                             // offset of the pair in a region plane
   const int oY = r * TX + 2 * lx;                         // offset of the pair in a y-push field
+  // region-plane offset of the ring column next to the pair for the lanes at the tile edge; one
+  // common (valid) word for all other lanes
+  const int eoff = lx == 0 ? oM - 1 : (lx == LX - 1 ? oM + 2 : RX + HL);
   const int ia = (tr - TY) * LX + lx;                     // aux thread index
   // x-exchange word of this lane: word (t & 31) of the y-push row owned by lane 0 of the warp
   const int trf = (t & ~31) / LX;
@@ -350,30 +353,33 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
           // a7: phi'(j) = inpl(j) + up(j-1)/8 + down(j+1)/8       (eqs. 23-24)
           phin = pfma(c_upa + down, T(0.125), c_inpl);
           // a5: kappa(j) = -div n from the z-combined normals a = S_z n_x, b = S_z n_y, c = d_z n_z
-          const T *za = s_zc + oM;
-          V own(T(0)), nb(T(0));
+          // Own columns from shared memory; the outer columns c0-1 / c0+2 come from the neighbour
+          // lanes by shuffle (3x the LSU rate, no bank conflicts).  The lanes at the tile edge read
+          // the ring column instead: one unconditional load per term through a per-lane pointer
+          // (all other lanes read one common word: a broadcast), no divergence.
+          const T *za = s_zc + oM, *zb = za + PL, *zc_ = za + 2 * PL;
+          V own(T(0)), eO(T(0));
 #pragma unroll
           for (int dy = -1; dy <= 1; ++dy) {
             const T w = dy == 0 ? w0 : w1;
-            own = pfma(lds_pair(za + dy * RX), w, own);
-            nb = pfma(V(za[dy * RX - 1], za[dy * RX + 2]), w, nb);
+            own = pfma(lds_pair(za + dy * RX), w, own);       // S_y a
+            eO = pfma(lds_pair(zc_ + dy * RX), w, eO);         // S_y c
           }
-          V kap(T(0.5) * (own.y - nb.x), T(0.5) * (nb.y - own.x));          // d/dx S_y a
-          const T *zb = za + PL;
-          const V dO = lds_pair(zb + RX) - lds_pair(zb - RX);
-          const V dN = V(zb[RX - 1], zb[RX + 2]) - V(zb[-RX - 1], zb[-RX + 2]);
-          kap.x += T(0.5) * (w1 * dN.x + w0 * dO.x + w1 * dO.y);            // S_x d/dy b
-          kap.y += T(0.5) * (w1 * dO.x + w0 * dO.y + w1 * dN.y);
-          const T *zc_ = za + 2 * PL;
-          V eO(T(0)), eN(T(0));
-#pragma unroll
-          for (int dy = -1; dy <= 1; ++dy) {
-            const T w = dy == 0 ? w0 : w1;
-            eO = pfma(lds_pair(zc_ + dy * RX), w, eO);
-            eN = pfma(V(zc_[dy * RX - 1], zc_[dy * RX + 2]), w, eN);
-          }
-          kap.x += w1 * eN.x + w0 * eO.x + w1 * eO.y;                        // S_x S_y c
-          kap.y += w1 * eO.x + w0 * eO.y + w1 * eN.y;
+          const V dO = lds_pair(zb + RX) - lds_pair(zb - RX);  // 2 d_y b
+          const T *ze = s_zc + eoff;                           // ring column (edge lanes) / dummy
+          const T ea = w1 * (ze[-RX] + ze[RX]) + w0 * ze[0];
+          const T ec = w1 * (ze[2 * PL - RX] + ze[2 * PL + RX]) + w0 * ze[2 * PL];
+          const T eb = ze[PL + RX] - ze[PL - RX];
+          auto left = [&](T v, T e) { const T q = __shfl_up_sync(0xffffffffu, v, 1, LX); return lx == 0 ? e : q; };
+          auto right = [&](T v, T e) { const T q = __shfl_down_sync(0xffffffffu, v, 1, LX); return lx == LX - 1 ? e : q; };
+          const T al = left(own.y, ea), ar = right(own.x, ea);
+          const T bl = left(dO.y, eb), br = right(dO.x, eb);
+          const T cl = left(eO.y, ec), cr = right(eO.x, ec);
+          V kap(T(0.5) * (own.y - al), T(0.5) * (ar - own.x));                     // d/dx S_y a
+          kap.x += T(0.5) * (w1 * bl + w0 * dO.x + w1 * dO.y);                       // S_x d/dy b
+          kap.y += T(0.5) * (w1 * dO.x + w0 * dO.y + w1 * br);
+          kap.x += w1 * cl + w0 * eO.x + w1 * eO.y;                                  // S_x S_y c
+          kap.y += w1 * eO.x + w0 * eO.y + w1 * cr;
           // a6: F = sigma kappa G, kappa = -div n, G = n (|G| + eps); u' = u_b + F / rho'
           const V sc = (kap * (gA + V(T(1e-12)))) * c_rinv * (-P.sigma);
           ukx = nA[0] * sc; uky = nA[1] * sc; ukz = nA[2] * sc;
