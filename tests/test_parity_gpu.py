@@ -363,9 +363,9 @@ def test_device_pointers_and_torch_stream():
 def test_warp_specialised_variant(monkeypatch):
     """tiled_ws_kernel (TSLB_WS=1: flow / phase / aux warps, setmaxnreg) computes the same step."""
     monkeypatch.setenv("TSLB_WS", "1")
-    prm = dict(nx=64, ny=32, nz=40, omega=1.9, two_component=True, sigma=0.01, interface_width=3.0)
-    d, r = oracle_run("ws-per", lambda: inputs.smooth_random(64, 32, 40, seed=8), prm, 10, tslb.F32)
-    g = tslb.Tslb(64, 32, 40, 1.9, precision=tslb.F32, kernel=tslb.KERNEL_TILED, **gpu_kwargs(prm))
+    prm = dict(nx=192, ny=24, nz=33, omega=1.9, two_component=True, sigma=0.01, interface_width=3.0)
+    d, r = oracle_run("tm%s" % ((192, 24, 33),), lambda: inputs.smooth_random(192, 24, 33, seed=5), prm, 10, tslb.F32)
+    g = tslb.Tslb(192, 24, 33, 1.9, precision=tslb.F32, kernel=tslb.KERNEL_TILED, **gpu_kwargs(prm))
     assert g.kernel_name.startswith("tiled-ws")
     g.init_fields(d["rho"], d["ux"], d["uy"], d["uz"], d["phi"], d["pineq"])
     g.step(10)
