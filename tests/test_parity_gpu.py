@@ -342,6 +342,11 @@ def test_state_roundtrip_and_errors():
         tslb.Tslb(16, 12, 10, 2.5)
     with pytest.raises(tslb.TslbError):
         tslb.Tslb(0, 12, 10, 1.0)
+    # kernel selection: AUTO takes the tiled kernel when the grid is a multiple of the tile, else generic
+    assert "tiled" in tslb.Tslb(64, 16, 4, 1.0).kernel_name
+    assert tslb.Tslb(48, 12, 10, 1.0).kernel_name == "generic"
+    with pytest.raises(tslb.TslbError):
+        tslb.Tslb(48, 12, 10, 1.0, kernel=tslb.KERNEL_TILED)
 
 
 def test_device_pointers_and_torch_stream():
