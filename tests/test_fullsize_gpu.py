@@ -99,3 +99,37 @@ def test_c5_full_size_sampled_against_oracle():
         assert v <= 1e-5, (k, v)
     assert bool(torch.isfinite(out["rho"]).all()) and bool(torch.isfinite(out["phi"]).all())
     sim.close()
+
+
+@pytest.mark.parametrize("We", [10.0, 200.0, 2000.0])
+def test_c4_jet_runs_stay_physical(We):
+    """BASELINE configs[3] at full size (256x256x512 fp32, D=20, U=0.05, Re=5000) for the three
+    Weber numbers, 2000 steps from rest: properties that hold at any size -- finite fields, phi in
+    [0,1] up to a small overshoot, density near 1, the jet tip advancing at about U/2 and the amount
+    of injected fluid matching the inlet flux  sum_nozzle U (1 + p xi) per step."""
+    import torch
+    nx, ny, nz, D, U = 256, 256, 512, 20, 0.05
+    prm = inputs.jet_params(nx, ny, nz, D, U=U, Re=5000.0, We=We, perturbation=0.05, seed=2024)
+    kw = {k: v for k, v in prm.items() if k not in ("nx", "ny", "nz", "omega")}
+    sim = tslb.Tslb(nx, ny, nz, prm["omega"], precision=tslb.F32, **kw)
+    dev = torch.device("cuda", 0)
+    one = torch.ones((nz, ny, nx), dtype=torch.float32, device=dev)
+    zero = torch.zeros((nz, ny, nx), dtype=torch.float32, device=dev)
+    sim.init_fields(one, zero, zero.clone(), zero.clone(), zero.clone())
+    steps = 2000
+    sim.step(steps)
+    m = sim.get_moments(device=True, want=("rho", "uz", "phi"))
+    rho, uz, phi = m["rho"], m["uz"], m["phi"]
+    assert bool(torch.isfinite(rho).all()) and bool(torch.isfinite(phi).all()) and bool(torch.isfinite(uz).all())
+    assert float(phi.min()) > -0.05 and float(phi.max()) < 1.05
+    assert 0.95 < float(rho.min()) and float(rho.max()) < 1.05
+    axis = phi[:, ny // 2 - 1:ny // 2 + 1, nx // 2 - 1:nx // 2 + 1].mean(dim=(1, 2)).cpu().numpy()
+    tip = int(np.argmax(axis < 0.5))
+    assert 0.3 * U * steps < tip < 1.2 * U * steps, tip
+    ndisc = sum(1 for x in range(nx) for y in range(ny)
+                if (2 * x - (nx - 1)) ** 2 + (2 * y - (ny - 1)) ** 2 < (2 * D / 2) ** 2)
+    injected = float(phi[1:].double().sum())
+    assert 0.6 * ndisc * U * steps < injected < 1.1 * ndisc * U * steps, (injected, ndisc * U * steps)
+    print("We", We, "tip", tip, "injected/expected", injected / (ndisc * U * steps),
+          "phi range", float(phi.min()), float(phi.max()), "rho range", float(rho.min()), float(rho.max()))
+    sim.close()
