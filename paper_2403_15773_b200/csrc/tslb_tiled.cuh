@@ -226,10 +226,6 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
   __syncthreads();
-  if (t == 0) {
-    issue(0);
-    if (NG > 1) issue(1);
-  }
 
   const V omc(P.omc);
   const T w1 = T(1.0 / 6.0), w0 = T(2.0 / 3.0);
@@ -278,16 +274,14 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
       }
     }
   };
-  if (!xrow) {
-    mbar_wait(&bars[0], 0u);
-    halo_cols(0);
-  }
-  __syncthreads();
-
-  int ms = 0, ps = 0, ns = 0;   // ring slots of this iteration: moments i%S, phi(k-1) i%SP, n(k) i%NR
-  for (int i = 0; i < NI; ++i) {
+  // Ring slots of iteration i: moments i%S, phi(k-1) i%SP, n(k) i%NR.  Iterations -2 and -1 are the
+  // pipeline prologue run through the same code (first two TMA groups, halo columns of the first
+  // plane): one copy of issue() and halo_cols() keeps the loop inside the instruction cache.
+  int ms = S - 2, ps = SP - 2, ns = NR - 2;
+  for (int i = -2; i < NI; ++i) {
     const int k = kb + i;
-    if (i < NG) mbar_wait(&bars[ms], (uint32_t)((i / S) & 1));
+    const bool act = (unsigned)i < (unsigned)NG;       // plane k is a source plane of this chunk
+    if (act) mbar_wait(&bars[ms], (uint32_t)((i / S) & 1));
     const int ms1 = ms == 0 ? S - 1 : ms - 1;          // moments of plane k-1
     const int ns1 = ns == 0 ? NR - 1 : ns - 1;         // n of plane k-1
     const int ns2 = ns1 == 0 ? NR - 1 : ns1 - 1;       // n of plane k-2
@@ -296,7 +290,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     const T *php = phi_at((ps + 2) % SP);              // phi(k+1)
 
     // =========================== segment 1 ===========================
-    if (TWO && !xrow && i < NG) {
+    if (TWO && !xrow && act) {
       // A1: T = S_y S_z phi, U = d_y S_z phi, V = S_y d_z phi of plane k on the region rows
       // one thread per column pair, marching down the rows with a 3-row window of S_z phi, d_z phi
       const int a1 = ia - 2 * LX;
@@ -410,7 +404,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
         }
       }
     }
-    if (xrow && i < NG) {
+    if (xrow && act) {
       // A2: x-pass of region row r of plane k in push form, then the y-push terms.  Each node's K is
       // evaluated once; a+ / a- cross to the x-neighbour thread through shared memory (same warp).
       V Xg[8][3];   // [group][p]
@@ -459,12 +453,12 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     if (t == 0 && i + 2 < NG) issue(i + 2);
 
     // =========================== segment 2 ===========================
-    if (!xrow && i + 1 < NG) {
+    if (!xrow && (unsigned)(i + 1) < (unsigned)NG) {
       const int sl = ms == S - 1 ? 0 : ms + 1;
       mbar_wait(&bars[sl], (uint32_t)(((i + 1) / S) & 1));
       halo_cols(sl);
     }
-    if (i < NG) {
+    if (act) {
       if (!aux) {
         // B2: finish the y-pass (a+ from the row below, a- from the row above, own a0) and z-push.
         V outm[10];
