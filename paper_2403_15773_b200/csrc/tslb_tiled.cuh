@@ -462,8 +462,6 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
       if (!aux) {
         // B2: finish the y-pass (a+ from the row below, a- from the row above, own a0) and z-push.
         V outm[10];
-#pragma unroll
-        for (int m = 0; m < 10; ++m) outm[m] = accA[m];
         // moment index of (p,q,rr)
         constexpr int MI[3][3][3] = {{{0, 3, 6}, {2, 9, -1}, {5, -1, -1}}, {{1, 8, -1}, {7, -1, -1}, {-1, -1, -1}}, {{4, -1, -1}, {-1, -1, -1}, {-1, -1, -1}}};
 #pragma unroll
@@ -481,15 +479,15 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
             push3<3, V, T>(Yq[q][0], Yq[q][1], Yq[q][2], ap, am, a0);   // ap -> plane k+1, am -> plane k-1
             {
               const int m = MI[p][q][0];
-              outm[m] = outm[m] + am; accA[m] = accB[m] + a0; accB[m] = ap;
+              outm[m] = accA[m] + am; accA[m] = accB[m] + a0; accB[m] = ap;
             }
             if (p + q <= 1) {
               const int m = MI[p][q][1];
-              outm[m] = outm[m] - am; accA[m] = accB[m]; accB[m] = ap;
+              outm[m] = accA[m] - am; accA[m] = accB[m]; accB[m] = ap;
             }
             if (p + q == 0) {
               const int m = MI[p][q][2];
-              outm[m] = pfma(am, T(2.0 / 3.0), outm[m]);
+              outm[m] = pfma(am, T(2.0 / 3.0), accA[m]);
               accA[m] = pfma(a0, T(-1.0 / 3.0), accB[m]);
               accB[m] = ap * T(2.0 / 3.0);
             }
