@@ -46,8 +46,10 @@ enum { TSLB_BC_PERIODIC = 0, TSLB_BC_JET_INFLOW = 1, TSLB_BC_OUTFLOW = 2 };
 enum {
   TSLB_KERNEL_AUTO = 0,     /* fastest kernel that supports the grid                           */
   TSLB_KERNEL_GENERIC = 1,  /* one thread per node, direct global loads; any grid size         */
-  TSLB_KERNEL_TILED = 2     /* TMA-staged x-y tiles marching along z; needs nx, ny multiples of
-                               the tile (tslb_create fails with TSLB_EINVAL otherwise)          */
+  TSLB_KERNEL_TILED = 2     /* TMA-staged 32x8 x-y tiles marching along z; needs nx >= 32, ny >= 8
+                               and nx a multiple of 4 (fp32) / 2 (fp64); a ragged last tile is
+                               shifted back inside the grid (tslb_create fails with TSLB_EINVAL
+                               when the grid is not supported)                                 */
 };
 
 typedef struct {

@@ -67,7 +67,7 @@ Validated validate(const tslb_params *p) {
   v.L = make_layout(p->nx, p->ny, p->nz);
   const bool tiled_ok = tiled_supported(p->precision, p->nx, p->ny, p->nz);
   if (p->kernel == TSLB_KERNEL_TILED && !tiled_ok)
-    return fail("TSLB_KERNEL_TILED needs nx and ny to be multiples of the tile (see tslb_tiled.cuh)");
+    return fail("TSLB_KERNEL_TILED needs nx >= 32, ny >= 8 and nx a multiple of 4 (fp32) or 2 (fp64)");
   v.kernel = (p->kernel == TSLB_KERNEL_GENERIC || !tiled_ok) ? TSLB_KERNEL_GENERIC : TSLB_KERNEL_TILED;
   // 2 buffers x nfields arrays, + 3 scratch arrays for the generic two-component path
   size_t narr = 2 * (size_t)v.nfields;
@@ -317,7 +317,8 @@ int tslb_create(const tslb_params *p, tslb_ctx **out) {
       delete c;
       return TSLB_ECUDA;
     }
-    if (p->precision == TSLB_F32 && p->two_component && TSLB_F32_TX == 32 && TSLB_TY == 8) {
+    if (p->precision == TSLB_F32 && p->two_component && TSLB_F32_TX == 32 && TSLB_TY == 8 && p->nx % 32 == 0 &&
+        p->ny % 8 == 0) {
       const char *env = getenv("TSLB_WS");
       c->use_ws = env ? atoi(env) != 0 : false;
     }

@@ -192,8 +192,10 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   // x-exchange word of this lane: word (t & 31) of the y-push row owned by lane 0 of the warp
   const int trf = (t & ~31) / LX;
   const int oX = (trf < TY ? trf + 1 : (trf == TY ? 0 : RY - 1)) * TX + (t & 31);
-  const int x0 = (blockIdx.x % M.ntx) * TX;
-  const int y0 = (blockIdx.x / M.ntx) * TY;
+  // Tile origin.  When nx (ny) is not a multiple of the tile, the last tile of the row (column) is
+  // shifted back to end at the domain edge; it recomputes the overlap but stores only its own nodes.
+  const int xs = (blockIdx.x % M.ntx) * TX, ys = (blockIdx.x / M.ntx) * TY;
+  const int x0 = min(xs, L.nx - TX), y0 = min(ys, L.ny - TY);
   const int z0 = blockIdx.y * M.zc;
   const int z1 = min(z0 + M.zc, L.nz);
   const int kb = z0 - 1;                 // first source plane
@@ -245,6 +247,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   const int gx_ = x0 + 2 * lx, gy_ = y0 + tr;
   const int gxg = gx_ < 2 ? gx_ + L.nx : (gx_ >= L.nx - 2 ? gx_ - L.nx : gx_);
   const int gyg = gy_ < GY ? gy_ + L.ny : (gy_ >= L.ny - GY ? gy_ - L.ny : gy_);
+  const bool own = gx_ >= xs && gy_ >= ys;
   const long long o00 = L.idx(gx_, gy_, 0), o10 = L.idx(gxg, gy_, 0), o01 = L.idx(gx_, gyg, 0), o11 = L.idx(gxg, gyg, 0);
 
   // x-pass terms of the two halo columns x0-1 (its a+) and x0+TX (its a-) of every region row of
@@ -380,7 +383,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
         }
         c_upa = c_upb; c_upb = up; c_inpl = inpl;
       }
-      if (fin && (P.zper || (j > 0 && j < L.nz - 1))) {
+      if (fin && own && (P.zper || (j > 0 && j < L.nz - 1))) {
         // a9: store plane j (and its periodic ghost images)
         V o[NF_MAX];
         o[0] = fl[0];
@@ -591,7 +594,8 @@ inline void tiled_tile(int precision, int &tx, int &ty) {
 inline bool tiled_supported(int precision, int nx, int ny, int nz) {
   int tx, ty;
   tiled_tile(precision, tx, ty);
-  return nx % tx == 0 && ny % ty == 0 && nz >= 1 && nx >= tx && ny >= ty;
+  // rows of the padded arrays must be multiples of 16 bytes for TMA (px = nx + 16)
+  return nx % (precision == TSLB_F32 ? 4 : 2) == 0 && nz >= 1 && nx >= tx && ny >= ty;
 }
 
 inline bool tiled_plan_create(TiledPlan &pl, int precision, const Layout &L, void *fields[2][NF_MAX], int nfields,
@@ -627,12 +631,12 @@ inline bool tiled_plan_create(TiledPlan &pl, int precision, const Layout &L, voi
     } else {
       pl.maps[b].phi = pl.maps[b].mom;
     }
-    pl.maps[b].ntx = L.nx / pl.tx;
-    pl.maps[b].nty = L.ny / pl.ty;
+    pl.maps[b].ntx = (L.nx + pl.tx - 1) / pl.tx;
+    pl.maps[b].nty = (L.ny + pl.ty - 1) / pl.ty;
   }
   // z chunking: every chunk pays a 3-plane pipeline prologue, and the grid runs in waves of
   // (CTAs per SM) x (SM count): pick the chunk length that minimises waves x (zc + 3).
-  const long long tiles = (long long)(L.nx / pl.tx) * (L.ny / pl.ty);
+  const long long tiles = (long long)pl.maps[0].ntx * pl.maps[0].nty;
   int nsm = 148;
   cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, device);
   const long long slots = (long long)nsm * (precision == TSLB_F32 ? 2 : 1);

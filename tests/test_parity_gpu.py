@@ -296,6 +296,21 @@ def test_tile_multiple_grids_with_ragged_z(kernel, shape):
     check("tm%s" % (shape,), lambda: inputs.smooth_random(nx, ny, nz, seed=5), prm, 10, tslb.F32, kernel)
 
 
+@pytest.mark.parametrize("shape", [(48, 12, 10), (100, 20, 6), (36, 9, 5), (72, 30, 19)])
+def test_ragged_tiles_tiled_kernel(shape):
+    """nx, ny not multiples of the 32x8 tile: the last tile is shifted back inside the grid."""
+    nx, ny, nz = shape
+    prm = dict(nx=nx, ny=ny, nz=nz, omega=1.8, two_component=True, sigma=0.01, interface_width=3.0)
+    check("rt%s" % (shape,), lambda: inputs.smooth_random(nx, ny, nz, seed=7), prm, 20, tslb.F64, tslb.KERNEL_TILED)
+    check("rt%s" % (shape,), lambda: inputs.smooth_random(nx, ny, nz, seed=7), prm, 10, tslb.F32, tslb.KERNEL_TILED)
+
+
+def test_production_shape_slab_400x400():
+    """The paper's production cross-section 400 x 400 (12.5 x 50 tiles) as a jet slab."""
+    prm = inputs.jet_params(400, 400, 12, D=20, U=0.05, Re=5000.0, We=200.0, perturbation=0.05, seed=3)
+    check("prod400", lambda: inputs.jet_developed(400, 400, 12, D=20, ndrop=2), prm, 4, tslb.F32, tslb.KERNEL_TILED)
+
+
 @pytest.mark.parametrize("kernel", KERNELS)
 def test_jet_small_ragged(kernel):
     prm = inputs.jet_params(64, 32, 11, D=9, U=0.04, Re=300.0, We=50.0, perturbation=0.1, seed=5)
@@ -342,11 +357,14 @@ def test_state_roundtrip_and_errors():
         tslb.Tslb(16, 12, 10, 2.5)
     with pytest.raises(tslb.TslbError):
         tslb.Tslb(0, 12, 10, 1.0)
-    # kernel selection: AUTO takes the tiled kernel when the grid is a multiple of the tile, else generic
+    # kernel selection: AUTO takes the tiled kernel when the grid holds a tile and its rows are
+    # TMA-aligned (ragged last tiles are fine), else generic
     assert "tiled" in tslb.Tslb(64, 16, 4, 1.0).kernel_name
-    assert tslb.Tslb(48, 12, 10, 1.0).kernel_name == "generic"
+    assert "tiled" in tslb.Tslb(48, 12, 10, 1.0).kernel_name
+    assert tslb.Tslb(46, 12, 10, 1.0, precision=tslb.F32).kernel_name == "generic"
+    assert tslb.Tslb(20, 12, 10, 1.0).kernel_name == "generic"
     with pytest.raises(tslb.TslbError):
-        tslb.Tslb(48, 12, 10, 1.0, kernel=tslb.KERNEL_TILED)
+        tslb.Tslb(20, 12, 10, 1.0, kernel=tslb.KERNEL_TILED)
 
 
 def test_device_pointers_and_torch_stream():
