@@ -26,7 +26,8 @@
  *   - All device work is enqueued on `stream`.  tslb_step() is asynchronous; tslb_get_moments()
  *     synchronises the stream before returning.
  *   - x and y are always periodic.  z is periodic, or jet inflow at z = 0 with outflow at
- *     z = nz-1 (eqs. 9-10, 223).
+ *     z = nz-1 (eqs. 9-10, 223); a z face can also be shared with another
+ *     context that holds the neighbouring z-slab (TSLB_BC_HALO, "z-slabs" below).
  */
 #ifndef TSLB_H
 #define TSLB_H
@@ -41,7 +42,11 @@ typedef struct tslb_ctx tslb_ctx; /* opaque, owned by the library */
 
 enum { TSLB_OK = 0, TSLB_EINVAL = -1, TSLB_ENOMEM = -2, TSLB_ECUDA = -3, TSLB_ESTATE = -4 };
 enum { TSLB_F32 = 0, TSLB_F64 = 1 };
-enum { TSLB_BC_PERIODIC = 0, TSLB_BC_JET_INFLOW = 1, TSLB_BC_OUTFLOW = 2 };
+/* z face types.  TSLB_BC_HALO marks a face shared with a neighbouring z-slab of a multi-GPU run
+ * (see "z-slabs" below): the context then keeps two ghost planes behind that face, which the
+ * neighbour fills.  Allowed pairs (zlo, zhi): PERIODIC/PERIODIC, JET_INFLOW/OUTFLOW, and with
+ * slabs HALO/HALO, JET_INFLOW/HALO, HALO/OUTFLOW.                                                */
+enum { TSLB_BC_PERIODIC = 0, TSLB_BC_JET_INFLOW = 1, TSLB_BC_OUTFLOW = 2, TSLB_BC_HALO = 3 };
 /* kernel selection (tslb_params.kernel) */
 enum {
   TSLB_KERNEL_AUTO = 0,     /* fastest kernel that supports the grid                           */
@@ -102,6 +107,42 @@ int tslb_step(tslb_ctx *c, int nsteps);
  * pointer (and any entry of pineq, or pineq itself) may be NULL.  Synchronises the stream.      */
 int tslb_get_moments(tslb_ctx *c, void *rho, void *ux, void *uy, void *uz, void *const pineq[6],
                      void *phi, int pointers_on_device);
+
+/* ---- z-slabs: one domain split along z over several contexts / GPUs (the paper's
+ * stated next step).  Every node update reads only time-t values within one
+ * plane (moments) / two planes (phi) of itself, so a slab needs, per step and per shared face, the
+ * neighbour's face plane of the 10 moments and its two planes of phi.  There is no exchange
+ * kernel and no pack/unpack: the step kernel of a slab stores those planes, besides its own
+ * time-t+1 buffer, straight into the neighbour's ghost planes through peer pointers (same process:
+ * the neighbour's workspace pointer; other process: a CUDA IPC handle of it; other GPU: NVLink
+ * peer stores).  Protocol (all slabs in lockstep):
+ *     create each slab with TSLB_BC_HALO on its shared faces, the same nx, ny, precision,
+ *     two_component and kernel; attach the neighbours; tslb_init_fields on every slab;
+ *     [barrier]  tslb_halo_push on every slab  [barrier]
+ *     repeat:  tslb_step(c, 1) on every slab;  [barrier: all slabs finished step t]
+ * The barrier must order the streams (same stream, an event, a tiny NCCL all-reduce on the
+ * stream, or a host barrier after a stream synchronise); tslb_step refuses nsteps > 1 on a slab.
+ * The inflow hash is keyed by (x, y, step) only, so a slab run reproduces the single-context run
+ * bit for bit.                                                                                    */
+
+/* Base device pointer of the context's workspace (to hand to a neighbour in the same process).  */
+void *tslb_workspace_ptr(const tslb_ctx *c);
+
+/* Declare the slab behind `face` (0: z low, 1: z high), whose workspace starts at device pointer
+ * nb_workspace (valid on this context's device: same device, peer-mapped, or IPC-opened) and
+ * which has nb_nz planes.  TSLB_EINVAL if the face is not a TSLB_BC_HALO face.  The pointer is
+ * kept until tslb_destroy; the neighbour must outlive this context's last step.                 */
+int tslb_attach_neighbor(tslb_ctx *c, int face, void *nb_workspace, int nb_nz);
+
+/* The same across processes: export this context's workspace as a 64-byte CUDA IPC handle (host
+ * buffer; needs a library-allocated workspace) / attach a neighbour from such a handle.         */
+int tslb_ipc_get_handle(tslb_ctx *c, void *handle64);
+int tslb_attach_neighbor_ipc(tslb_ctx *c, int face, const void *handle64, int nb_nz);
+
+/* Copy the face planes of the CURRENT buffer into the attached neighbours' ghost planes
+ * (asynchronous on the stream).  Needed once after tslb_init_fields; afterwards tslb_step keeps
+ * the ghost planes current by itself.                                                           */
+int tslb_halo_push(tslb_ctx *c);
 
 /* Number of time steps taken since tslb_init_fields (keys the inflow hash).                     */
 long long tslb_step_count(const tslb_ctx *c);

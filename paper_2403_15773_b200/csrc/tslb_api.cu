@@ -24,20 +24,35 @@ thread_local std::string g_create_error;
 
 size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
-Layout make_layout(int nx, int ny, int nz) {
+Layout make_layout(int nx, int ny, int nz, int gz) {
   Layout L;
   L.nx = nx; L.ny = ny; L.nz = nz;
   L.px = nx + 2 * GX;
   L.py = ny + 2 * GY;
+  L.gz = gz;
   L.plane = (long long)L.px * L.py;
-  L.field = (long long)round_up((size_t)L.plane * nz, 64);
+  L.field = (long long)round_up((size_t)L.plane * (nz + 2 * gz), 64);
   return L;
+}
+
+// Carving of a workspace into the 2 x nfields field arrays; the pointers are those of plane 0 (after
+// the gz ghost planes).  The same function locates a NEIGHBOUR slab's arrays from its workspace base.
+void carve_fields(void *ws, const Layout &L, size_t esize, int nfields, void *fields[2][NF_MAX], size_t *end) {
+  const size_t fb = round_up((size_t)L.field * esize, 256);
+  const size_t z0 = (size_t)L.gz * (size_t)L.plane * esize;
+  char *base = (char *)ws;
+  size_t off = 0;
+  for (int b = 0; b < 2; ++b)
+    for (int k = 0; k < nfields; ++k) { fields[b][k] = base + off + z0; off += fb; }
+  if (end) *end = off;
 }
 
 struct Validated {
   bool ok = false;
   std::string why;
   bool zper = true;
+  bool slab = false;                  // at least one z face is a halo face
+  bool halo_lo = false, halo_hi = false, jet_lo = false, out_hi = false;
   int kernel = TSLB_KERNEL_GENERIC;   // resolved kernel
   size_t esize = 4;
   int nfields = 10;
@@ -57,14 +72,25 @@ Validated validate(const tslb_params *p) {
   if (p->two_component && !(p->interface_width > 0.0)) return fail("interface_width must be > 0 when two_component");
   const bool zper = p->bc_zlo == TSLB_BC_PERIODIC && p->bc_zhi == TSLB_BC_PERIODIC;
   const bool jet = p->bc_zlo == TSLB_BC_JET_INFLOW && p->bc_zhi == TSLB_BC_OUTFLOW;
-  if (!zper && !jet) return fail("boundary types must be PERIODIC/PERIODIC or JET_INFLOW/OUTFLOW");
-  if (jet && p->nz < 4) return fail("nz >= 4 is required with inflow/outflow");
-  if (jet && !(p->jet_diameter >= 0.0)) return fail("jet_diameter must be >= 0");
+  v.halo_lo = p->bc_zlo == TSLB_BC_HALO;
+  v.halo_hi = p->bc_zhi == TSLB_BC_HALO;
+  v.slab = v.halo_lo || v.halo_hi;
+  v.jet_lo = p->bc_zlo == TSLB_BC_JET_INFLOW;
+  v.out_hi = p->bc_zhi == TSLB_BC_OUTFLOW;
+  if (v.slab) {
+    if (!(v.halo_lo || v.jet_lo) || !(v.halo_hi || v.out_hi))
+      return fail("a slab face is TSLB_BC_HALO, or JET_INFLOW (z low) / OUTFLOW (z high)");
+    if (p->nz < 2) return fail("a slab needs nz >= 2 (the halo is two planes deep)");
+  } else {
+    if (!zper && !jet) return fail("boundary types must be PERIODIC/PERIODIC or JET_INFLOW/OUTFLOW (or TSLB_BC_HALO faces)");
+    if (jet && p->nz < 4) return fail("nz >= 4 is required with inflow/outflow");
+  }
+  if ((v.jet_lo || v.out_hi) && !(p->jet_diameter >= 0.0)) return fail("jet_diameter must be >= 0");
   if (p->kernel < TSLB_KERNEL_AUTO || p->kernel > TSLB_KERNEL_TILED) return fail("unknown kernel selector");
   v.zper = zper;
   v.esize = p->precision == TSLB_F32 ? 4 : 8;
   v.nfields = p->two_component ? 11 : 10;
-  v.L = make_layout(p->nx, p->ny, p->nz);
+  v.L = make_layout(p->nx, p->ny, p->nz, v.slab ? GZ : 0);
   const bool tiled_ok = tiled_supported(p->precision, p->nx, p->ny, p->nz);
   if (p->kernel == TSLB_KERNEL_TILED && !tiled_ok)
     return fail("TSLB_KERNEL_TILED needs nx >= 32, ny >= 8 and nx a multiple of 4 (fp32) or 2 (fp64)");
@@ -87,6 +113,11 @@ struct tslb_ctx {
   bool own_ws = false;
   void *fields[2][NF_MAX] = {};
   void *nrm[3] = {};
+  void *nb_fields[2][2][NF_MAX] = {};   // [side][buffer][field]: neighbour slabs' arrays (peer pointers)
+  int nb_nz[2] = {0, 0};
+  bool nb_on[2] = {false, false};
+  void *nb_ipc[2] = {nullptr, nullptr}; // bases opened with cudaIpcOpenMemHandle
+  unsigned char nb_handle[2][64] = {};
   int cur = 0;                 // index of the buffer holding time t
   bool inited = false;
   long long t = 0;
@@ -132,6 +163,12 @@ StepParams<T> make_step_params(tslb_ctx *c, int src, int dst) {
   P.sigma = (T)(c->p.two_component ? c->p.sigma : 0.0);
   P.gamma = (T)(c->p.two_component ? 2.0 / c->p.interface_width : 0.0);
   P.zper = c->v.zper ? 1 : 0;
+  P.halo_lo = c->v.halo_lo; P.halo_hi = c->v.halo_hi;
+  P.jet_lo = c->v.jet_lo; P.out_hi = c->v.out_hi;
+  for (int side = 0; side < 2; ++side) {
+    for (int k = 0; k < NF_MAX; ++k) P.nb[side].f[k] = c->nb_on[side] ? (T *)c->nb_fields[side][dst][k] : nullptr;
+    P.nb_dz[side] = side == 0 ? c->nb_nz[0] : -c->v.L.nz;
+  }
   P.jetD2 = c->p.jet_diameter * c->p.jet_diameter;
   P.jetU = (T)c->p.jet_velocity;
   P.jetP = (T)c->p.jet_perturbation;
@@ -145,7 +182,7 @@ int launch_generic(tslb_ctx *c, const StepParams<T> &P) {
   const Layout &L = P.L;
   const bool two = c->p.two_component != 0;
   if (two) {
-    dim3 b(32, 8), g((L.nx + 31) / 32, (L.ny + 7) / 8, L.nz);
+    dim3 b(32, 8), g((L.nx + 31) / 32, (L.ny + 7) / 8, L.nz + (P.halo_lo ? 1 : 0) + (P.halo_hi ? 1 : 0));
     phase_normals_kernel<T><<<g, b, 0, c->stream>>>(P);
     c->launches++;
   }
@@ -176,7 +213,7 @@ int step_typed(tslb_ctx *c, int nsteps) {
       } else {
         e = launch_tiled<T>(c->tiled, P, c->cur, c->p.hermite_order, c->p.two_component != 0, c->stream);
       }
-      c->launches += c->v.zper ? 1 : 2;   // + the boundary-plane kernel with inflow/outflow
+      c->launches += (c->v.jet_lo || c->v.out_hi) ? 2 : 1;   // + the boundary-plane kernel with inflow/outflow
       rc = (e == cudaSuccess) ? TSLB_OK : c->cuda_fail(e, "launch_tiled");
     } else {
       rc = launch_generic<T>(c, P);
@@ -218,7 +255,7 @@ int init_typed(tslb_ctx *c, const void *const src[NF_MAX], int on_device) {
   }
   c->cur = 0;
   c->t = 0;
-  if (!c->v.zper) {
+  if (c->v.jet_lo || c->v.out_hi) {
     StepParams<T> P = make_step_params<T>(c, 0, 0);
     dim3 gb((L.nx + 127) / 128, L.ny, 2);
     boundary_init_kernel<T><<<gb, b, 0, c->stream>>>(P, c->p.two_component);
@@ -227,8 +264,14 @@ int init_typed(tslb_ctx *c, const void *const src[NF_MAX], int on_device) {
   int rc = fill_all_ghosts<T>(c, 0);
   if (rc != TSLB_OK) return rc;
   // the other buffer's ghosts/halo start from a defined state too
-  for (int k = 0; k < c->v.nfields; ++k)
-    CK(cudaMemsetAsync(c->fields[1][k], 0, (size_t)L.field * sizeof(T), c->stream));
+  const size_t zb = (size_t)L.gz * (size_t)L.plane * sizeof(T);
+  for (int k = 0; k < c->v.nfields; ++k) {
+    CK(cudaMemsetAsync((char *)c->fields[1][k] - zb, 0, (size_t)L.field * sizeof(T), c->stream));
+    if (zb) {   // ghost planes of the current buffer: defined until the neighbours push theirs
+      CK(cudaMemsetAsync((char *)c->fields[0][k] - zb, 0, zb, c->stream));
+      CK(cudaMemsetAsync((char *)c->fields[0][k] + (size_t)L.plane * L.nz * sizeof(T), 0, zb, c->stream));
+    }
+  }
   CK(cudaStreamSynchronize(c->stream));
   return TSLB_OK;
 }
@@ -305,10 +348,9 @@ int tslb_create(const tslb_params *p, tslb_ctx **out) {
   const size_t fb = round_up((size_t)v.L.field * v.esize, 256);
   char *base = (char *)c->ws;
   size_t off = 0;
-  for (int b = 0; b < 2; ++b)
-    for (int k = 0; k < v.nfields; ++k) { c->fields[b][k] = base + off; off += fb; }
+  carve_fields(c->ws, v.L, v.esize, v.nfields, c->fields, &off);
   if (v.kernel == TSLB_KERNEL_GENERIC && p->two_component)
-    for (int k = 0; k < 3; ++k) { c->nrm[k] = base + off; off += fb; }
+    for (int k = 0; k < 3; ++k) { c->nrm[k] = base + off + (size_t)v.L.gz * v.L.plane * v.esize; off += fb; }
   if (v.kernel == TSLB_KERNEL_TILED) {
     std::string why;
     if (!tiled_plan_create(c->tiled, p->precision, v.L, c->fields, v.nfields, p->device, why)) {
@@ -318,7 +360,7 @@ int tslb_create(const tslb_params *p, tslb_ctx **out) {
       return TSLB_ECUDA;
     }
     if (p->precision == TSLB_F32 && p->two_component && TSLB_F32_TX == 32 && TSLB_TY == 8 && p->nx % 32 == 0 &&
-        p->ny % 8 == 0) {
+        p->ny % 8 == 0 && !v.slab) {
       const char *env = getenv("TSLB_WS");
       c->use_ws = env ? atoi(env) != 0 : false;
     }
@@ -355,6 +397,11 @@ int tslb_step(tslb_ctx *c, int nsteps) {
   if (!c) return TSLB_EINVAL;
   if (nsteps < 0) return c->fail(TSLB_EINVAL, "nsteps must be >= 0");
   if (!c->inited) return c->fail(TSLB_ESTATE, "tslb_step before tslb_init_fields");
+  if (c->v.slab && nsteps > 1)
+    return c->fail(TSLB_EINVAL, "a slab advances one step per call: its neighbours must finish step t before step t+1 starts");
+  for (int side = 0; side < 2; ++side)
+    if ((side == 0 ? c->v.halo_lo : c->v.halo_hi) && !c->nb_on[side] && nsteps > 0)
+      return c->fail(TSLB_ESTATE, "halo face %d has no neighbour attached (tslb_attach_neighbor)", side);
   CK(cudaSetDevice(c->p.device));
   return c->p.precision == TSLB_F32 ? step_typed<float>(c, nsteps) : step_typed<double>(c, nsteps);
 }
@@ -375,6 +422,82 @@ int tslb_get_moments(tslb_ctx *c, void *rho, void *ux, void *uy, void *uz, void 
     for (int k = 0; k < 6; ++k) dst[F_PXX + k] = pineq[k];
   return c->p.precision == TSLB_F32 ? get_typed<float>(c, dst, pointers_on_device)
                                     : get_typed<double>(c, dst, pointers_on_device);
+}
+
+void *tslb_workspace_ptr(const tslb_ctx *c) { return c ? c->ws : nullptr; }
+
+int tslb_attach_neighbor(tslb_ctx *c, int face, void *nb_workspace, int nb_nz) {
+  if (!c) return TSLB_EINVAL;
+  if (face != 0 && face != 1) return c->fail(TSLB_EINVAL, "face must be 0 (z low) or 1 (z high)");
+  if (!(face == 0 ? c->v.halo_lo : c->v.halo_hi)) return c->fail(TSLB_EINVAL, "face %d is not a TSLB_BC_HALO face", face);
+  if (!nb_workspace || nb_nz < 2) return c->fail(TSLB_EINVAL, "neighbour workspace is NULL or its nz < 2");
+  // a neighbour on another device of this process: map it (NVLink peer access)
+  cudaPointerAttributes at;
+  if (cudaPointerGetAttributes(&at, nb_workspace) == cudaSuccess && at.type == cudaMemoryTypeDevice &&
+      at.device != c->p.device) {
+    CK(cudaSetDevice(c->p.device));
+    cudaError_t e = cudaDeviceEnablePeerAccess(at.device, 0);
+    if (e == cudaErrorPeerAccessAlreadyEnabled) { cudaGetLastError(); e = cudaSuccess; }
+    if (e != cudaSuccess) return c->cuda_fail(e, "cudaDeviceEnablePeerAccess");
+  } else {
+    cudaGetLastError();
+  }
+  const Layout Ln = make_layout(c->p.nx, c->p.ny, nb_nz, GZ);
+  carve_fields(nb_workspace, Ln, c->v.esize, c->v.nfields, c->nb_fields[face], nullptr);
+  c->nb_nz[face] = nb_nz;
+  c->nb_on[face] = true;
+  return TSLB_OK;
+}
+
+int tslb_ipc_get_handle(tslb_ctx *c, void *handle64) {
+  if (!c || !handle64) return TSLB_EINVAL;
+  static_assert(sizeof(cudaIpcMemHandle_t) == 64, "handle size");
+  if (!c->own_ws) return c->fail(TSLB_ESTATE, "IPC export needs a workspace allocated by tslb_create");
+  CK(cudaSetDevice(c->p.device));
+  cudaIpcMemHandle_t h;
+  CK(cudaIpcGetMemHandle(&h, c->ws));
+  memcpy(handle64, &h, 64);
+  return TSLB_OK;
+}
+
+int tslb_attach_neighbor_ipc(tslb_ctx *c, int face, const void *handle64, int nb_nz) {
+  if (!c || !handle64) return TSLB_EINVAL;
+  if (face != 0 && face != 1) return c->fail(TSLB_EINVAL, "face must be 0 (z low) or 1 (z high)");
+  CK(cudaSetDevice(c->p.device));
+  cudaIpcMemHandle_t h;
+  memcpy(&h, handle64, 64);
+  // two slabs with periodic z: both faces see the same neighbour -- open its handle once
+  const int other = face ^ 1;
+  if (c->nb_ipc[other] && memcmp(c->nb_handle[other], handle64, 64) == 0)
+    return tslb_attach_neighbor(c, face, c->nb_ipc[other], nb_nz);
+  void *base = nullptr;
+  CK(cudaIpcOpenMemHandle(&base, h, cudaIpcMemLazyEnablePeerAccess));
+  int rc = tslb_attach_neighbor(c, face, base, nb_nz);
+  if (rc != TSLB_OK) { cudaIpcCloseMemHandle(base); return rc; }
+  if (c->nb_ipc[face]) cudaIpcCloseMemHandle(c->nb_ipc[face]);
+  c->nb_ipc[face] = base;
+  memcpy(c->nb_handle[face], handle64, 64);
+  return TSLB_OK;
+}
+
+int tslb_halo_push(tslb_ctx *c) {
+  if (!c) return TSLB_EINVAL;
+  if (!c->inited) return c->fail(TSLB_ESTATE, "tslb_halo_push before tslb_init_fields");
+  CK(cudaSetDevice(c->p.device));
+  const Layout &L = c->v.L;
+  const size_t pb = (size_t)L.plane * c->v.esize;
+  for (int side = 0; side < 2; ++side) {
+    if (!c->nb_on[side]) continue;
+    for (int k = 0; k < c->v.nfields; ++k) {
+      // my planes 0,1 -> the lower neighbour's planes nz', nz'+1; my planes nz-2, nz-1 -> the upper
+      // neighbour's planes -2, -1 (padded planes are contiguous, ghost columns included)
+      const char *src = (const char *)c->fields[c->cur][k] + (side == 0 ? 0 : (size_t)(L.nz - 2) * pb);
+      char *dst = (char *)c->nb_fields[side][c->cur][k];
+      if (side == 0) dst += (size_t)c->nb_nz[0] * pb; else dst -= 2 * pb;
+      CK(cudaMemcpyAsync(dst, src, 2 * pb, cudaMemcpyDefault, c->stream));
+    }
+  }
+  return TSLB_OK;
 }
 
 long long tslb_step_count(const tslb_ctx *c) { return c ? c->t : -1; }
@@ -402,6 +525,8 @@ int tslb_destroy(tslb_ctx *c) {
   cudaSetDevice(c->p.device);
   cudaStreamSynchronize(c->stream);
   tiled_plan_destroy(c->tiled);
+  for (int side = 0; side < 2; ++side)
+    if (c->nb_ipc[side]) cudaIpcCloseMemHandle(c->nb_ipc[side]);
   if (c->stage) cudaFree(c->stage);
   if (c->own_ws && c->ws) cudaFree(c->ws);
   delete c;

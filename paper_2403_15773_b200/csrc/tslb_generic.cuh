@@ -11,9 +11,6 @@
 namespace tslb {
 
 __device__ __forceinline__ int wrapi(int i, int n) { return i < 0 ? i + n : (i >= n ? i - n : i); }
-__device__ __forceinline__ int mapz(int z, int nz, int zper) {
-  return zper ? wrapi(z, nz) : (z < 0 ? 0 : (z >= nz ? nz - 1 : z));
-}
 
 template <typename T> __device__ __forceinline__ T eps_n() { return T(1e-12); }
 template <typename T> __device__ __forceinline__ T tsqrt(T x);
@@ -23,12 +20,13 @@ template <> __device__ __forceinline__ double tsqrt<double>(double x) { return s
 // G = (1/c_s^2) sum_i w_i c_i phi(x + c_i)  (eqs. 20-21, readings A6/A7) in
 // its separable form: central difference along one axis, [1/6,2/3,1/6] along the other two.
 template <typename T>
-__device__ __forceinline__ void grad_phi(const T *__restrict__ phi, const Layout &L, int x, int y, int z,
-                                         int zper, T G[3]) {
+__device__ __forceinline__ void grad_phi(const T *__restrict__ phi, const StepParams<T> &P, int x, int y, int z,
+                                         T G[3]) {
+  const Layout &L = P.L;
   T gx = 0, gy = 0, gz = 0;
 #pragma unroll
   for (int dz = -1; dz <= 1; ++dz) {
-    const int zz = mapz(z + dz, L.nz, zper);
+    const int zz = zsrc(P, z + dz);
 #pragma unroll
     for (int dy = -1; dy <= 1; ++dy) {
       const int yy = wrapi(y + dy, L.ny);
@@ -51,10 +49,10 @@ __global__ void __launch_bounds__(256) phase_normals_kernel(const __grid_constan
   const Layout &L = P.L;
   const int x = blockIdx.x * blockDim.x + threadIdx.x;
   const int y = blockIdx.y * blockDim.y + threadIdx.y;
-  const int z = blockIdx.z;
+  const int z = (int)blockIdx.z - (P.halo_lo ? 1 : 0);   // slab: n is needed on one ghost plane per halo face
   if (x >= L.nx || y >= L.ny) return;
   T G[3];
-  grad_phi<T>(P.in.f[F_PHI], L, x, y, z, P.zper, G);
+  grad_phi<T>(P.in.f[F_PHI], P, x, y, z, G);
   const T mag = tsqrt<T>(G[0] * G[0] + G[1] * G[1] + G[2] * G[2]);
   const T inv = T(1) / (mag + eps_n<T>());
   const long long i = L.idx(x, y, z);
@@ -98,7 +96,7 @@ __global__ void __launch_bounds__(128) generic_step_kernel(const __grid_constant
   const long long i0 = L.idx(x, y, z);
   constexpr int NF = TWO ? 11 : 10;
 
-  if (!P.zper && (z == 0 || z == L.nz - 1)) {
+  if ((P.jet_lo && z == 0) || (P.out_hi && z == L.nz - 1)) {
     T o[NF_MAX];
     boundary_node<T>(P, P.in, x, y, z, P.step_next, o, TWO);
 #pragma unroll
@@ -113,7 +111,7 @@ __global__ void __launch_bounds__(128) generic_step_kernel(const __grid_constant
   for (int k = 0; k < 10; ++k) M[k] = T(0);
 #pragma unroll
   for (int cz = -1; cz <= 1; ++cz) {
-    const int zz = mapz(z - cz, L.nz, P.zper);
+    const int zz = zsrc(P, z - cz);
 #pragma unroll
     for (int cy = -1; cy <= 1; ++cy) {
       const int yy = wrapi(y - cy, L.ny);
@@ -148,11 +146,11 @@ __global__ void __launch_bounds__(128) generic_step_kernel(const __grid_constant
   if (TWO) {
     // a5: G at the node from the OLD phi; kappa = -(1/c_s^2) sum_i w_i c_i . n(x + c_i)
     T G[3];
-    grad_phi<T>(P.in.f[F_PHI], L, x, y, z, P.zper, G);
+    grad_phi<T>(P.in.f[F_PHI], P, x, y, z, G);
     T div = T(0);
 #pragma unroll
     for (int dz = -1; dz <= 1; ++dz) {
-      const int zz = mapz(z + dz, L.nz, P.zper);
+      const int zz = zsrc(P, z + dz);
 #pragma unroll
       for (int dy = -1; dy <= 1; ++dy) {
         const int yy = wrapi(y + dy, L.ny);
@@ -178,7 +176,7 @@ __global__ void __launch_bounds__(128) generic_step_kernel(const __grid_constant
     T acc = T(0.25) * pc;
     const int xm = wrapi(x - 1, L.nx), xp = wrapi(x + 1, L.nx);
     const int ym = wrapi(y - 1, L.ny), yp = wrapi(y + 1, L.ny);
-    const int zm = mapz(z - 1, L.nz, P.zper), zp = mapz(z + 1, L.nz, P.zper);
+    const int zm = zsrc(P, z - 1), zp = zsrc(P, z + 1);
     const long long jn[6] = {L.idx(xm, y, z), L.idx(xp, y, z), L.idx(x, ym, z),
                              L.idx(x, yp, z), L.idx(x, y, zm), L.idx(x, y, zp)};
     // neighbour at x - c_i: c_i = +e for the "minus" neighbour, -e for the "plus" neighbour
@@ -201,6 +199,24 @@ __global__ void __launch_bounds__(128) generic_step_kernel(const __grid_constant
 #pragma unroll
   for (int k = 0; k < 6; ++k) P.out.f[F_PXX + k][i0] = pin[k];
   if (TWO) P.out.f[F_PHI][i0] = phin;
+  // halo push into the neighbour slabs' ghost planes (interior nodes; this path never reads ghost
+  // columns).  Slab face planes that are jet boundary planes have no neighbour.
+#pragma unroll
+  for (int side = 0; side < 2; ++side) {
+    if (!P.nb[side].f[0]) continue;
+    const int depth = side == 0 ? z : L.nz - 1 - z;     // 0: face plane, 1: the plane behind it
+    if (depth > 1) continue;
+    const long long i1 = L.idx(x, y, z + P.nb_dz[side]);
+    if (depth == 0) {
+      P.nb[side].f[F_DRHO][i1] = drho;
+      P.nb[side].f[F_UX][i1] = ub[0];
+      P.nb[side].f[F_UY][i1] = ub[1];
+      P.nb[side].f[F_UZ][i1] = ub[2];
+#pragma unroll
+      for (int k = 0; k < 6; ++k) P.nb[side].f[F_PXX + k][i1] = pin[k];
+    }
+    if (TWO) P.nb[side].f[F_PHI][i1] = phin;
+  }
 }
 
 // ---- layout conversion / ghost maintenance / boundary init -------------------------------
@@ -249,6 +265,7 @@ __global__ void boundary_init_kernel(const __grid_constant__ StepParams<T> P, in
   const int y = blockIdx.y;
   const int z = blockIdx.z ? L.nz - 1 : 0;
   if (x >= L.nx) return;
+  if (blockIdx.z ? !P.out_hi : !P.jet_lo) return;
   T o[NF_MAX];
   boundary_node<T>(P, P.out, x, y, z, 0, o, two != 0);
   const long long i0 = L.idx(x, y, z);

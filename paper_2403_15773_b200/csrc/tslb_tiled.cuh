@@ -154,7 +154,9 @@ __device__ __forceinline__ void pull3s(T l, T upy, T dnx, T r, V a0, V &W0, V &W
 }
 
 // ------------------------------------------------------------------ the kernel
-template <typename T, int TX, int TY, int ORDER, bool TWO>
+// SLAB: the context is a z-slab (halo faces, ghost planes, halo push).  A separate instantiation:
+// the single-GPU kernel's loop body sits at the 32 KB instruction-cache limit and must not grow.
+template <typename T, int TX, int TY, int ORDER, bool TWO, bool SLAB>
 __global__ void __launch_bounds__((TX / 2) * (TY + 4), (TileCfg<T, TX, TY, TWO>::SMEM_BYTES <= 113 * 1024 ? 2 : 1))
 tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant__ TiledMaps M) {
   using C = TileCfg<T, TX, TY, TWO>;
@@ -202,10 +204,9 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   const int NG = z1 - kb + 1;            // load groups / x-pass planes: kb .. z1
   const int NI = NG + 1;                 // iterations
 
-  auto zmap = [&](int z) {
-    if (P.zper) { z %= L.nz; return z < 0 ? z + L.nz : z; }
-    return z < 0 ? 0 : (z >= L.nz ? L.nz - 1 : z);
-  };
+  // plane coordinate in the tensor map: wrapped / clamped / ghost plane of a slab (zsrc), shifted
+  // by the ghost planes below z = 0
+  auto zmap = [&](int z) { return zsrc(P, z) + L.gz; };
   // group g (relative index): moments of plane kb+g -> slot g%S, phi of plane kb+g+1 -> slot (g+2)%SP
   auto issue = [&](int g) {
     uint64_t *bar = &bars[g % S];
@@ -281,10 +282,11 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   // pipeline prologue run through the same code (first two TMA groups, halo columns of the first
   // plane): one copy of issue() and halo_cols() keeps the loop inside the instruction cache.
   int ms = S - 2, ps = SP - 2, ns = NR - 2;
+  uint32_t mph = 1;                      // mbarrier phase parity of slot ms (flips when ms wraps to 0)
   for (int i = -2; i < NI; ++i) {
     const int k = kb + i;
     const bool act = (unsigned)i < (unsigned)NG;       // plane k is a source plane of this chunk
-    if (act) mbar_wait(&bars[ms], (uint32_t)((i / S) & 1));
+    if (act) mbar_wait(&bars[ms], mph);
     const int ms1 = ms == 0 ? S - 1 : ms - 1;          // moments of plane k-1
     const int ns1 = ns == 0 ? NR - 1 : ns - 1;         // n of plane k-1
     const int ns2 = ns1 == 0 ? NR - 1 : ns1 - 1;       // n of plane k-2
@@ -383,7 +385,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
         }
         c_upa = c_upb; c_upb = up; c_inpl = inpl;
       }
-      if (fin && own && (P.zper || (j > 0 && j < L.nz - 1))) {
+      if (fin && own && !((P.jet_lo && j == 0) || (P.out_hi && j == L.nz - 1))) {
         // a9: store plane j (and its periodic ghost images)
         V o[NF_MAX];
         o[0] = fl[0];
@@ -395,13 +397,30 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
 #pragma unroll
         for (int m = 0; m < (TWO ? 11 : 10); ++m) *reinterpret_cast<V *>(P.out.f[m] + zo + o00) = o[m];
         if (gxg != gx_ || gyg != gy_) {          // periodic ghost images (edge tiles only)
+#pragma unroll 1
+          for (int im = 0; im < 3; ++im) {       // one copy of the store code: x image, y image, corner
+            if (im == 0 ? gxg == gx_ : (im == 1 ? gyg == gy_ : (gxg == gx_ || gyg == gy_))) continue;
+            const long long og = zo + (im == 0 ? o10 : (im == 1 ? o01 : o11));
 #pragma unroll
-          for (int m = 0; m < (TWO ? 11 : 10); ++m) {
-            T *base = P.out.f[m] + zo;
-            if (gxg != gx_) *reinterpret_cast<V *>(base + o10) = o[m];
-            if (gyg != gy_) {
-              *reinterpret_cast<V *>(base + o01) = o[m];
-              if (gxg != gx_) *reinterpret_cast<V *>(base + o11) = o[m];
+            for (int m = 0; m < (TWO ? 11 : 10); ++m) *reinterpret_cast<V *>(P.out.f[m] + og) = o[m];
+          }
+        }
+        // halo push (slab faces only, off the common path): the same stores into the neighbour
+        // slab's ghost planes through its peer pointers -- phi from the two planes next to the
+        // face, the moments from the face plane
+        if (SLAB && ((j < 2 && P.nb[0].f[0]) || (j >= L.nz - 2 && P.nb[1].f[0]))) {
+#pragma unroll 1
+          for (int side = 0; side < 2; ++side) {
+            const int depth = side == 0 ? j : L.nz - 1 - j;
+            if (!P.nb[side].f[0] || depth > 1) continue;
+            const long long zn = (long long)(j + P.nb_dz[side]) * L.plane;
+#pragma unroll 1
+            for (int im = 0; im < 4; ++im) {     // the node itself, then its x / y / corner images
+              if (im == 1 ? gxg == gx_ : (im == 2 ? gyg == gy_ : (im == 3 && (gxg == gx_ || gyg == gy_)))) continue;
+              const long long og = zn + (im == 0 ? o00 : (im == 1 ? o10 : (im == 2 ? o01 : o11)));
+#pragma unroll
+              for (int m = 0; m < (TWO ? 11 : 10); ++m)
+                if (depth == 0 || m == F_PHI) *reinterpret_cast<V *>(P.nb[side].f[m] + og) = o[m];
             }
           }
         }
@@ -458,7 +477,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     // =========================== segment 2 ===========================
     if (!xrow && (unsigned)(i + 1) < (unsigned)NG) {
       const int sl = ms == S - 1 ? 0 : ms + 1;
-      mbar_wait(&bars[sl], (uint32_t)(((i + 1) / S) & 1));
+      mbar_wait(&bars[sl], sl == 0 ? mph ^ 1u : mph);
       halo_cols(sl);
     }
     if (act) {
@@ -558,6 +577,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     }
     __syncthreads();
     ms = ms == S - 1 ? 0 : ms + 1;
+    if (ms == 0) mph ^= 1u;
     ps = ps == SP - 1 ? 0 : ps + 1;
     ns = ns == NR - 1 ? 0 : ns + 1;
   }
@@ -616,16 +636,17 @@ inline bool tiled_plan_create(TiledPlan &pl, int precision, const Layout &L, voi
   const int RX = pl.tx + 2 * (es == 4 ? 4 : 2), RY = pl.ty + 2, RYP = pl.ty + 4;
   for (int b = 0; b < 2; ++b) {
     const size_t fstride = (size_t)((char *)fields[b][1] - (char *)fields[b][0]);
-    cuuint64_t gdim[4] = {(cuuint64_t)L.px, (cuuint64_t)L.py, (cuuint64_t)L.nz, 10};
+    cuuint64_t gdim[4] = {(cuuint64_t)L.px, (cuuint64_t)L.py, (cuuint64_t)(L.nz + 2 * L.gz), 10};
+    const size_t zoff = (size_t)L.gz * (size_t)L.plane * es;     // fields[][] point at plane 0
     cuuint64_t gstr[3] = {(cuuint64_t)L.px * es, (cuuint64_t)L.plane * es, (cuuint64_t)fstride};
     cuuint32_t box[4] = {(cuuint32_t)RX, (cuuint32_t)RY, 1, 10};
     cuuint32_t estr[4] = {1, 1, 1, 1};
-    CUresult r = enc(&pl.maps[b].mom, dt, 4, fields[b][0], gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+    CUresult r = enc(&pl.maps[b].mom, dt, 4, (char *)fields[b][0] - zoff, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                      CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) { why = "cuTensorMapEncodeTiled(moments) failed: " + std::to_string((int)r); return false; }
     if (pl.two) {
       cuuint32_t boxp[3] = {(cuuint32_t)RX, (cuuint32_t)RYP, 1};
-      r = enc(&pl.maps[b].phi, dt, 3, fields[b][F_PHI], gdim, gstr, boxp, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+      r = enc(&pl.maps[b].phi, dt, 3, (char *)fields[b][F_PHI] - zoff, gdim, gstr, boxp, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
       if (r != CUDA_SUCCESS) { why = "cuTensorMapEncodeTiled(phi) failed: " + std::to_string((int)r); return false; }
     } else {
@@ -666,6 +687,7 @@ __global__ void tiled_boundary_kernel(const __grid_constant__ StepParams<T> P, i
   const int Y = blockIdx.y;
   const int z = blockIdx.z ? L.nz - 1 : 0;
   if (X >= L.px) return;
+  if (blockIdx.z ? !P.out_hi : !P.jet_lo) return;
   const int x = ((X - GX) % L.nx + L.nx) % L.nx, y = ((Y - GY) % L.ny + L.ny) % L.ny;
   T o[NF_MAX];
   boundary_node<T>(P, P.in, x, y, z, P.step_next, o, two != 0);
@@ -676,13 +698,14 @@ __global__ void tiled_boundary_kernel(const __grid_constant__ StepParams<T> P, i
 
 template <typename T, int TX, int TY>
 cudaError_t launch_tiled_t(TiledPlan &pl, const StepParams<T> &P, int src, int order, bool two, cudaStream_t st) {
+  const bool slab = P.halo_lo || P.halo_hi;
   const TiledMaps &M = pl.maps[src];
   dim3 grid(M.ntx * M.nty, (P.L.nz + M.zc - 1) / M.zc);
   cudaError_t e = cudaSuccess;
-#define TSLB_LAUNCH(ORD, TWOC)                                                                        \
+#define TSLB_LAUNCH(ORD, TWOC, SL)                                                                      \
   do {                                                                                                \
     using Cf = TileCfg<T, TX, TY, TWOC>;                                                              \
-    auto kern = tiled_step_kernel<T, TX, TY, ORD, TWOC>;                                              \
+    auto kern = tiled_step_kernel<T, TX, TY, ORD, TWOC, SL>;                                          \
     static bool attr_set = false;                                                                     \
     if (!attr_set) {                                                                                  \
       e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cf::SMEM_BYTES); \
@@ -691,12 +714,17 @@ cudaError_t launch_tiled_t(TiledPlan &pl, const StepParams<T> &P, int src, int o
     }                                                                                                 \
     kern<<<grid, Cf::NTHREADS, Cf::SMEM_BYTES, st>>>(P, M);                                           \
   } while (0)
-  if (two) { if (order >= 3) TSLB_LAUNCH(3, true); else TSLB_LAUNCH(2, true); }
-  else     { if (order >= 3) TSLB_LAUNCH(3, false); else TSLB_LAUNCH(2, false); }
+  if (slab) {
+    if (two) { if (order >= 3) TSLB_LAUNCH(3, true, true); else TSLB_LAUNCH(2, true, true); }
+    else     { if (order >= 3) TSLB_LAUNCH(3, false, true); else TSLB_LAUNCH(2, false, true); }
+  } else {
+    if (two) { if (order >= 3) TSLB_LAUNCH(3, true, false); else TSLB_LAUNCH(2, true, false); }
+    else     { if (order >= 3) TSLB_LAUNCH(3, false, false); else TSLB_LAUNCH(2, false, false); }
+  }
 #undef TSLB_LAUNCH
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  if (!P.zper) {
+  if (P.jet_lo || P.out_hi) {
     dim3 b(128), g((P.L.px + 127) / 128, P.L.py, 2);
     tiled_boundary_kernel<T><<<g, b, 0, st>>>(P, two ? 1 : 0);
     e = cudaGetLastError();

@@ -75,7 +75,7 @@ tiled_ws_kernel(const __grid_constant__ StepParams<float> P, const __grid_consta
   const int NI = NG + 1;
 
   auto zmap = [&](int z) {
-    if (P.zper) { z %= L.nz; return z < 0 ? z + L.nz : z; }
+    if (P.zper) { while (z < 0) z += L.nz; while (z >= L.nz) z -= L.nz; return z; }
     return z < 0 ? 0 : (z >= L.nz ? L.nz - 1 : z);
   };
   auto issue = [&](int g) {

@@ -14,12 +14,13 @@ _SO = os.path.join(_HERE, "libtslb.so")
 
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
 F32, F64 = 0, 1
-BC_PERIODIC, BC_JET_INFLOW, BC_OUTFLOW = 0, 1, 2
+BC_PERIODIC, BC_JET_INFLOW, BC_OUTFLOW, BC_HALO = 0, 1, 2, 3
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED = 0, 1, 2
 
 EXPORTS = ["tslb_workspace_bytes", "tslb_create", "tslb_init_fields", "tslb_step",
            "tslb_get_moments", "tslb_step_count", "tslb_kernel_name", "tslb_launch_count",
-           "tslb_debug_xi", "tslb_destroy", "tslb_last_error"]
+           "tslb_debug_xi", "tslb_destroy", "tslb_last_error", "tslb_workspace_ptr",
+           "tslb_attach_neighbor", "tslb_ipc_get_handle", "tslb_attach_neighbor_ipc", "tslb_halo_push"]
 
 
 class Params(ctypes.Structure):
@@ -74,6 +75,12 @@ def lib():
         L.tslb_destroy.argtypes = [vp]
         L.tslb_last_error.argtypes = [vp]
         L.tslb_last_error.restype = ctypes.c_char_p
+        L.tslb_workspace_ptr.argtypes = [vp]
+        L.tslb_workspace_ptr.restype = vp
+        L.tslb_attach_neighbor.argtypes = [vp, ctypes.c_int, vp, ctypes.c_int]
+        L.tslb_ipc_get_handle.argtypes = [vp, vp]
+        L.tslb_attach_neighbor_ipc.argtypes = [vp, ctypes.c_int, vp, ctypes.c_int]
+        L.tslb_halo_push.argtypes = [vp]
         _lib = L
     return _lib
 
@@ -81,10 +88,12 @@ def lib():
 def make_params(nx, ny, nz, omega, precision=F32, two_component=False, hermite_order=3, sigma=0.0,
                 interface_width=4.0, jet=False, jet_diameter=0.0, jet_velocity=0.0,
                 jet_perturbation=0.0, seed=0, device=0, kernel=KERNEL_AUTO, stream=None,
-                workspace=None, workspace_bytes=0):
+                workspace=None, workspace_bytes=0, bc_zlo=None, bc_zhi=None):
+    """`jet` sets JET_INFLOW/OUTFLOW; bc_zlo / bc_zhi override one face (BC_HALO for a z-slab)."""
+    lo = (BC_JET_INFLOW if jet else BC_PERIODIC) if bc_zlo is None else bc_zlo
+    hi = (BC_OUTFLOW if jet else BC_PERIODIC) if bc_zhi is None else bc_zhi
     return Params(nx, ny, nz, precision, int(bool(two_component)), hermite_order, omega, sigma,
-                  interface_width, BC_JET_INFLOW if jet else BC_PERIODIC,
-                  BC_OUTFLOW if jet else BC_PERIODIC, jet_diameter, jet_velocity, jet_perturbation,
+                  interface_width, lo, hi, jet_diameter, jet_velocity, jet_perturbation,
                   seed, device, kernel, stream, workspace, workspace_bytes)
 
 
@@ -208,6 +217,28 @@ class Tslb:
             out["pineq"] = torch.stack(comps) if device else np.stack(comps)
         out["phi"] = phi
         return out
+
+    # -- z-slabs (include/tslb.h "z-slabs")
+    @property
+    def workspace_ptr(self):
+        return lib().tslb_workspace_ptr(self._h)
+
+    def attach_neighbor(self, face, other):
+        """Same process: `other` is the Tslb holding the slab behind `face` (0: z low, 1: z high)."""
+        self._check(lib().tslb_attach_neighbor(self._h, int(face), other.workspace_ptr, other.shape[0]))
+
+    def ipc_handle(self):
+        """64-byte CUDA IPC handle of the workspace (needs torch_workspace=False)."""
+        buf = ctypes.create_string_buffer(64)
+        self._check(lib().tslb_ipc_get_handle(self._h, buf))
+        return buf.raw
+
+    def attach_neighbor_ipc(self, face, handle, nb_nz):
+        buf = ctypes.create_string_buffer(bytes(handle), 64)
+        self._check(lib().tslb_attach_neighbor_ipc(self._h, int(face), buf, int(nb_nz)))
+
+    def halo_push(self):
+        self._check(lib().tslb_halo_push(self._h))
 
     # -- bookkeeping / probes
     @property
