@@ -144,6 +144,19 @@ int tslb_attach_neighbor_ipc(tslb_ctx *c, int face, const void *handle64, int nb
  * the ghost planes current by itself.                                                           */
 int tslb_halo_push(tslb_ctx *c);
 
+/* ---- time averages on the mid x-z plane (Figs. 5-6: the time-averaged phase
+ * field and axial velocity, from which the centre-line 1/<phi_c>, 1/<u_c> and the radial profiles
+ * follow).  After tslb_stats_begin(c, every), every `every`-th time step adds phi and u_z of the
+ * plane y = (ny-1)/2 (the mean of the two middle rows when ny is even: the jet axis lies between
+ * them) to fp64 running sums, by a small kernel on the context's stream.  tslb_stats_get copies
+ * the sums (HOST pointers, nx*nz doubles each, element (x,z) at x + nx*z; either may be NULL;
+ * sum_phi is left untouched when !two_component) and the number of samples; <q> = sum / nsamples.
+ * tslb_stats_begin again restarts the sums; tslb_stats_end stops accumulating.  A z-slab
+ * accumulates its own planes.                                                                    */
+int tslb_stats_begin(tslb_ctx *c, int every);
+int tslb_stats_get(tslb_ctx *c, double *sum_phi, double *sum_uz, long long *nsamples);
+int tslb_stats_end(tslb_ctx *c);
+
 /* Number of time steps taken since tslb_init_fields (keys the inflow hash).                     */
 long long tslb_step_count(const tslb_ctx *c);
 

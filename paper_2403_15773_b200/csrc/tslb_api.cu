@@ -123,6 +123,9 @@ struct tslb_ctx {
   long long t = 0;
   long long launches = 0;
   void *stage = nullptr;       // one dense field, for host <-> device import/export
+  double *stat = nullptr;      // mid-plane running sums: [0] phi, [1] u_z, nx*nz doubles each
+  int stat_every = 0;          // 0: off
+  long long stat_n = 0;        // samples accumulated
   TiledPlan tiled;             // TMA descriptors etc.
   bool use_ws = false;         // warp-specialised variant of the tiled kernel (fp32, two-component)
   std::string err;
@@ -221,6 +224,17 @@ int step_typed(tslb_ctx *c, int nsteps) {
     if (rc != TSLB_OK) return rc;
     c->cur ^= 1;
     c->t++;
+    if (c->stat_every && c->t % c->stat_every == 0) {
+      const Layout &L = c->v.L;
+      const size_t n = (size_t)L.nx * L.nz;
+      dim3 b(128), g((L.nx + 127) / 128, L.nz);
+      plane_stats_kernel<T><<<g, b, 0, c->stream>>>(L, c->p.two_component ? (const T *)c->fields[c->cur][F_PHI] : nullptr,
+                                                   (const T *)c->fields[c->cur][F_UZ], (L.ny - 1) / 2, L.ny / 2, c->stat,
+                                                   c->stat + n);
+      CK(cudaGetLastError());
+      c->launches++;
+      c->stat_n++;
+    }
   }
   return TSLB_OK;
 }
@@ -500,6 +514,39 @@ int tslb_halo_push(tslb_ctx *c) {
   return TSLB_OK;
 }
 
+int tslb_stats_begin(tslb_ctx *c, int every) {
+  if (!c) return TSLB_EINVAL;
+  if (every < 1) return c->fail(TSLB_EINVAL, "every must be >= 1");
+  CK(cudaSetDevice(c->p.device));
+  const size_t n = (size_t)c->p.nx * c->p.nz;
+  if (!c->stat) {
+    cudaError_t e = cudaMalloc((void **)&c->stat, 2 * n * sizeof(double));
+    if (e != cudaSuccess) return c->fail(TSLB_ENOMEM, "cudaMalloc(stats): %s", cudaGetErrorString(e));
+  }
+  CK(cudaMemsetAsync(c->stat, 0, 2 * n * sizeof(double), c->stream));
+  c->stat_every = every;
+  c->stat_n = 0;
+  return TSLB_OK;
+}
+
+int tslb_stats_get(tslb_ctx *c, double *sum_phi, double *sum_uz, long long *nsamples) {
+  if (!c) return TSLB_EINVAL;
+  if (!c->stat) return c->fail(TSLB_ESTATE, "tslb_stats_get before tslb_stats_begin");
+  CK(cudaSetDevice(c->p.device));
+  const size_t n = (size_t)c->p.nx * c->p.nz;
+  if (sum_phi) CK(cudaMemcpyAsync(sum_phi, c->stat, n * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  if (sum_uz) CK(cudaMemcpyAsync(sum_uz, c->stat + n, n * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  if (nsamples) *nsamples = c->stat_n;
+  return TSLB_OK;
+}
+
+int tslb_stats_end(tslb_ctx *c) {
+  if (!c) return TSLB_EINVAL;
+  c->stat_every = 0;
+  return TSLB_OK;
+}
+
 long long tslb_step_count(const tslb_ctx *c) { return c ? c->t : -1; }
 const char *tslb_kernel_name(const tslb_ctx *c) { return c ? c->kname.c_str() : ""; }
 long long tslb_launch_count(const tslb_ctx *c) { return c ? c->launches : -1; }
@@ -528,6 +575,7 @@ int tslb_destroy(tslb_ctx *c) {
   for (int side = 0; side < 2; ++side)
     if (c->nb_ipc[side]) cudaIpcCloseMemHandle(c->nb_ipc[side]);
   if (c->stage) cudaFree(c->stage);
+  if (c->stat) cudaFree(c->stat);
   if (c->own_ws && c->ws) cudaFree(c->ws);
   delete c;
   return TSLB_OK;

@@ -273,6 +273,21 @@ __global__ void boundary_init_kernel(const __grid_constant__ StepParams<T> P, in
   for (int k = 0; k < nf; ++k) P.out.f[k][i0] = o[k];
 }
 
+// Running sums for the time averages <phi>, <u_z> on the mid x-z plane (Figs. 5-6;
+// SURVEY NEXT-3).  The jet axis is at y = (ny-1)/2: rows y0 = floor, y1 = ceil of it are averaged.
+// One thread per (x, z); fp64 accumulators; traffic 2 rows per plane, negligible beside the step.
+template <typename T>
+__global__ void plane_stats_kernel(Layout L, const T *__restrict__ phi, const T *__restrict__ uz, int y0, int y1,
+                                   double *__restrict__ sum_phi, double *__restrict__ sum_uz) {
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  const int z = blockIdx.y;
+  if (x >= L.nx) return;
+  const long long i0 = L.idx(x, y0, z), i1 = L.idx(x, y1, z);
+  const long long o = (long long)z * L.nx + x;
+  sum_uz[o] += 0.5 * ((double)uz[i0] + (double)uz[i1]);
+  if (phi) sum_phi[o] += 0.5 * ((double)phi[i0] + (double)phi[i1]);
+}
+
 template <typename T>
 __global__ void debug_xi_kernel(unsigned long long seed, int nx, int ny, long long step, double *out) {
   const int x = blockIdx.x * blockDim.x + threadIdx.x;

@@ -20,7 +20,8 @@ KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED = 0, 1, 2
 EXPORTS = ["tslb_workspace_bytes", "tslb_create", "tslb_init_fields", "tslb_step",
            "tslb_get_moments", "tslb_step_count", "tslb_kernel_name", "tslb_launch_count",
            "tslb_debug_xi", "tslb_destroy", "tslb_last_error", "tslb_workspace_ptr",
-           "tslb_attach_neighbor", "tslb_ipc_get_handle", "tslb_attach_neighbor_ipc", "tslb_halo_push"]
+           "tslb_attach_neighbor", "tslb_ipc_get_handle", "tslb_attach_neighbor_ipc", "tslb_halo_push",
+           "tslb_stats_begin", "tslb_stats_get", "tslb_stats_end"]
 
 
 class Params(ctypes.Structure):
@@ -81,6 +82,9 @@ def lib():
         L.tslb_ipc_get_handle.argtypes = [vp, vp]
         L.tslb_attach_neighbor_ipc.argtypes = [vp, ctypes.c_int, vp, ctypes.c_int]
         L.tslb_halo_push.argtypes = [vp]
+        L.tslb_stats_begin.argtypes = [vp, ctypes.c_int]
+        L.tslb_stats_get.argtypes = [vp, vp, vp, ctypes.POINTER(ctypes.c_longlong)]
+        L.tslb_stats_end.argtypes = [vp]
         _lib = L
     return _lib
 
@@ -239,6 +243,23 @@ class Tslb:
 
     def halo_push(self):
         self._check(lib().tslb_halo_push(self._h))
+
+    # -- time averages on the mid x-z plane (include/tslb.h)
+    def stats_begin(self, every=1):
+        self._check(lib().tslb_stats_begin(self._h, int(every)))
+
+    def stats_get(self):
+        """-> dict(phi=<phi>(z,x) or None, uz=<u_z>(z,x), nsamples): time averages so far."""
+        nz, ny, nx = self.shape
+        sp = np.zeros((nz, nx), dtype=np.float64)
+        su = np.zeros((nz, nx), dtype=np.float64)
+        n = ctypes.c_longlong(0)
+        self._check(lib().tslb_stats_get(self._h, sp.ctypes.data if self.two else None, su.ctypes.data, ctypes.byref(n)))
+        k = max(1, n.value)
+        return dict(phi=sp / k if self.two else None, uz=su / k, nsamples=n.value)
+
+    def stats_end(self):
+        self._check(lib().tslb_stats_end(self._h))
 
     # -- bookkeeping / probes
     @property
