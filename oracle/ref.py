@@ -15,6 +15,7 @@ _SO = os.path.join(_HERE, "libtslb_ref.so")
 _SRC = [os.path.join(_HERE, "tslb_ref.cpp"), os.path.join(_HERE, "tslb_ref.h")]
 
 BC_PERIODIC, BC_JET_INFLOW, BC_OUTFLOW = 0, 1, 2
+FORCING_KICK, FORCING_GUO = 0, 1
 
 
 def build(force=False):
@@ -37,6 +38,7 @@ class _Params(ctypes.Structure):
         ("jet_diameter", ctypes.c_double), ("jet_velocity", ctypes.c_double),
         ("jet_perturbation", ctypes.c_double),
         ("seed", ctypes.c_ulonglong),
+        ("forcing", ctypes.c_int),
     ]
 
 
@@ -64,6 +66,8 @@ def lib():
         L.tslb_ref_fneq.restype = None
         L.tslb_ref_get_populations.argtypes = [ctypes.c_void_p, _dp]
         L.tslb_ref_phase_geometry.argtypes = [ctypes.c_void_p, _dp, _dp, _dp, _dp]
+        L.tslb_ref_set_extra_force.argtypes = [ctypes.c_void_p, _dp]
+        L.tslb_ref_get_physical_velocity.argtypes = [ctypes.c_void_p, _dp, _dp, _dp]
         L.tslb_ref_xi.argtypes = [ctypes.c_ulonglong, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                   ctypes.c_int, ctypes.c_longlong]
         L.tslb_ref_xi.restype = ctypes.c_double
@@ -114,13 +118,13 @@ class Oracle:
 
     def __init__(self, nx, ny, nz, omega, two_component=False, hermite_order=3, sigma=0.0,
                  interface_width=4.0, bc_zlo=BC_PERIODIC, bc_zhi=BC_PERIODIC, jet_diameter=0.0,
-                 jet_velocity=0.0, jet_perturbation=0.0, seed=0):
+                 jet_velocity=0.0, jet_perturbation=0.0, seed=0, forcing=FORCING_KICK):
         self.shape = (nz, ny, nx)
         self.N = nx * ny * nz
         self.two = bool(two_component)
         self._prm = _Params(nx, ny, nz, int(self.two), hermite_order, omega, sigma,
                             interface_width, bc_zlo, bc_zhi, jet_diameter, jet_velocity,
-                            jet_perturbation, seed)
+                            jet_perturbation, seed, int(forcing))
         self._h = ctypes.c_void_p()
         rc = lib().tslb_ref_create(ctypes.byref(self._prm), ctypes.byref(self._h))
         if rc != 0:
@@ -169,6 +173,24 @@ class Oracle:
         if rc != 0:
             raise RuntimeError("tslb_ref_get_moments failed: %d" % rc)
         return dict(rho=rho, ux=ux, uy=uy, uz=uz, pineq=pin, phi=phi)
+
+    def set_extra_force(self, F):
+        """Pin-only probe: static force density F (3, nz, ny, nx) added to sigma kappa grad(phi);
+        None clears it.  Call before init_fields."""
+        if F is None:
+            rc = lib().tslb_ref_set_extra_force(self._h, None)
+        else:
+            F = _c64(F)
+            assert F.shape == (3,) + self.shape
+            rc = lib().tslb_ref_set_extra_force(self._h, _p(F))
+        assert rc == 0
+
+    def get_physical_velocity(self):
+        """-> (3, nz, ny, nx): the time-centred velocity (KICK: u' - F/2rho; GUO: u_b + F/2rho)."""
+        u = np.empty((3,) + self.shape)
+        rc = lib().tslb_ref_get_physical_velocity(self._h, _p(u[0]), _p(u[1]), _p(u[2]))
+        assert rc == 0
+        return u
 
     def get_populations(self):
         f = np.empty((27,) + self.shape)

@@ -141,6 +141,11 @@ struct tslb_ref_ctx {
   std::vector<double> rho, u, pineq, phi;   /* N, 3N, 6N, N  (time-t fields)     */
   std::vector<double> rho2, u2, pineq2, phi2;
   std::vector<double> G, nrm, kappa;        /* 3N, 3N, N (phase geometry, old phi) */
+  std::vector<double> Fext;                 /* 3N or empty: pin-only extra force density      */
+  std::vector<double> Ftot;                 /* 3N: KICK: force of the last kick; GUO: force of
+                                               the current fields (the one in fpost)          */
+  std::vector<double> drho_s;               /* N (GUO): rho - 1 exactly as the moment sum gave it */
+  bool guo;
 
   inline int wrapx(int x) const { return (x % p.nx + p.nx) % p.nx; }
   inline int wrapy(int y) const { return (y % p.ny + p.ny) % p.ny; }
@@ -196,6 +201,70 @@ struct tslb_ref_ctx {
     for (int q = 0; q < 27; ++q) dst[(size_t)q * N + i] = fe[q] + (1.0 - p.omega) * fn[q];
   }
 
+  /* Force density of the CURRENT fields: F = sigma kappa G (eq. 20, A6/A7) from the
+   * current phi [+ the pin-only extra force]; zero on inflow/outflow planes (their moments are
+   * imposed, O9).  Also leaves n of the current phi in nrm. */
+  void compute_force() {
+    const bool two = p.two_component != 0;
+    if (two) phase_geometry();
+    for (int a = 0; a < 3; ++a)
+      for (size_t i = 0; i < N; ++i) {
+        double F = two ? p.sigma * kappa[i] * G[a * N + i] : 0.0;
+        if (!Fext.empty()) F += Fext[a * N + i];
+        Ftot[a * N + i] = F;
+      }
+    if (!zper)
+      for (int a = 0; a < 3; ++a)
+        for (int y = 0; y < p.ny; ++y)
+          for (int x = 0; x < p.nx; ++x)
+            Ftot[a * N + idx(x, y, 0)] = Ftot[a * N + idx(x, y, p.nz - 1)] = 0.0;
+  }
+
+  /* Reading A18: collision with the forcing of Guo, Zheng & Shi (2002).  From the
+   * bare moments rho, u_b = m/rho, Pi_b^neq = Pi - rho c_s^2 delta - rho u_b u_b of the streamed
+   * populations and the force F of the same time level:
+   *   u      = u_b + F / (2 rho)                                  (Guo eq. 19: rho u = m + F/2)
+   *   Pi^neq = Pi - rho c_s^2 delta - rho u u                     (second moment of f - f^eq(u);
+   *            Guo's (uF + Fu)/2 belongs to the viscous-stress diagnostic, not to the relaxation)
+   *   f^pre  = f^eq(rho,u) + f^neq(Pi^neq,u) + w_i c_i.(m - rho u)/c_s^2,   m - rho u = -F/2
+   *            (regularized pre-collision state, eqs. 16/19 + the first-order Hermite term that
+   *            carries the momentum defect of f^eq(u))
+   *   f^post = f^eq + (1-omega)(f^pre - f^eq) + (1 - omega/2) S_i                (Guo eq. 4, 20)
+   *   S_i    = w_i [ (c_i - u).F / c_s^2 + (c_i.u)(c_i.F) / c_s^4 ]
+   * With F = 0 this is collide_node bit for bit. */
+  void collide_guo(size_t i, double drho, const double ub[3], const double pn[6], const double F[3],
+                   double *dst) const {
+    const double rho = 1.0 + drho;
+    double uu[3], a2b[3][3], a2[3][3], fe[27], fn[27];
+    for (int a = 0; a < 3; ++a) uu[a] = ub[a] + F[a] / (2.0 * rho);
+    sym6_to_33(pn, a2b);
+    for (int a = 0; a < 3; ++a)
+      for (int b = 0; b < 3; ++b)
+        a2[a][b] = a2b[a][b] + (rho * ub[a] * ub[b] - rho * uu[a] * uu[b]);
+    feq_dev(drho, uu, p.hermite_order, fe);
+    fneq(a2, uu, p.hermite_order, fn);
+    double uF = 0.0;
+    for (int a = 0; a < 3; ++a) uF += uu[a] * F[a];
+    for (int q = 0; q < 27; ++q) {
+      double cF = 0.0, cu = 0.0;
+      for (int a = 0; a < 3; ++a) { cF += L.c[q][a] * F[a]; cu += L.c[q][a] * uu[a]; }
+      const double first = L.w[q] * (-0.5 * cF) / CS2;
+      const double S = L.w[q] * ((cF - uF) / CS2 + cu * cF / (CS2 * CS2));
+      dst[(size_t)q * N + i] = fe[q] + (1.0 - p.omega) * (fn[q] + first) + (1.0 - 0.5 * p.omega) * S;
+    }
+  }
+
+  void collide_all_guo() {
+#pragma omp parallel for schedule(static)
+    for (long long i = 0; i < (long long)N; ++i) {
+      const double ub[3] = {u[i], u[N + i], u[2 * N + i]};
+      const double F[3] = {Ftot[i], Ftot[N + i], Ftot[2 * N + i]};
+      double pn[6];
+      for (int k = 0; k < 6; ++k) pn[k] = pineq[k * N + i];
+      collide_guo((size_t)i, drho_s[i], ub, pn, F, fpost.data());
+    }
+  }
+
   /* O9: moments imposed on the two z boundary planes, from time-t ("old") fields in r,uo,po,ph
    * (eqs. 9-10; A10, A11).  step_index keys the inflow hash. */
   void boundary_planes(const std::vector<double> &r, const std::vector<double> &uo,
@@ -240,7 +309,10 @@ struct tslb_ref_ctx {
   void step_once() {
     const int nx = p.nx, ny = p.ny, nz = p.nz;
     const bool two = p.two_component != 0;
-    if (two) phase_geometry(); /* O5, from OLD phi */
+    const bool forced = two || !Fext.empty();
+    /* KICK: O5, force and n from the OLD phi.  GUO: Ftot and nrm already belong to the current
+     * (time-t) fields -- they were formed for the collision that produced fpost. */
+    if (!guo) compute_force();
 #pragma omp parallel for schedule(static)
     for (int z = 0; z < nz; ++z) {
       if (is_boundary(z)) continue; /* overwritten in O9; their pulled values are never used */
@@ -273,11 +345,13 @@ struct tslb_ref_ctx {
               a2[a][b] = P[a][b] - rh * ub[a] * ub[b] - ((a == b) ? drho * CS2 : 0.0);
           /* O5/O6 force and kick                              PAPER.md:192 eq. 20; A9 */
           double un[3] = {ub[0], ub[1], ub[2]};
-          if (two)
-            for (int a = 0; a < 3; ++a) un[a] += p.sigma * kappa[i] * G[a * N + i] / rh;
-          /* O2+O3+O7 collide                                  PAPER.md:91 eq. 5 */
+          if (forced && !guo)
+            for (int a = 0; a < 3; ++a) un[a] += Ftot[a * N + i] / rh;
+          /* O2+O3+O7 collide                                  PAPER.md:91 eq. 5
+           * (GUO: the bare moments are stored; the collision follows once F(t+1) is known) */
           const double pn[6] = {a2[0][0], a2[1][1], a2[2][2], a2[0][1], a2[0][2], a2[1][2]};
-          collide_node(i, drho, un, pn, fpost2.data());
+          if (!guo) collide_node(i, drho, un, pn, fpost2.data());
+          else drho_s[i] = drho;
           rho2[i] = rh;
           for (int a = 0; a < 3; ++a) u2[a * N + i] = un[a];
           for (int k = 0; k < 6; ++k) pineq2[k * N + i] = pn[k];
@@ -288,7 +362,11 @@ struct tslb_ref_ctx {
               size_t j = idx(wrapx(x - L.c7[q][0]), wrapy(y - L.c7[q][1]), mapz(z - L.c7[q][2]));
               double cu = 0.0, cn = 0.0;
               for (int a = 0; a < 3; ++a) {
-                cu += L.c7[q][a] * u[a * N + j];
+                /* advecting velocity: the stored one (KICK, A9) / the time-centred physical
+                 * velocity u_b + F/(2 rho) of the source node (GUO, A18) */
+                double ua = u[a * N + j];
+                if (guo) ua += Ftot[a * N + j] / (2.0 * rho[j]);
+                cu += L.c7[q][a] * ua;
                 cn += L.c7[q][a] * nrm[a * N + j];
               }
               double ph = phi[j];
@@ -299,10 +377,20 @@ struct tslb_ref_ctx {
         }
     }
     if (!zper) boundary_planes(rho, u, pineq, phi, rho2, u2, pineq2, phi2, fpost2, t + 1);
-    fpost.swap(fpost2);
+    if (!guo) fpost.swap(fpost2);
     rho.swap(rho2); u.swap(u2); pineq.swap(pineq2);
     if (two) phi.swap(phi2);
     ++t;
+    if (guo) {
+      if (!zper)
+        for (int y = 0; y < ny; ++y)
+          for (int x = 0; x < nx; ++x) {
+            drho_s[idx(x, y, 0)] = rho[idx(x, y, 0)] - 1.0;
+            drho_s[idx(x, y, nz - 1)] = rho[idx(x, y, nz - 1)] - 1.0;
+          }
+      compute_force();     /* F(t+1), n(t+1) from the new phi */
+      collide_all_guo();   /* fpost(t+1), boundary planes included (F = 0 there) */
+    }
   }
 };
 
@@ -319,6 +407,7 @@ int tslb_ref_create(const tslb_ref_params *p, tslb_ref_ctx **out) {
   bool jet = (p->bc_zlo == TSLB_REF_BC_JET_INFLOW && p->bc_zhi == TSLB_REF_BC_OUTFLOW);
   if (!zper && !jet) return -1;
   if (jet && p->nz < 4) return -1;
+  if (p->forcing != TSLB_REF_FORCING_KICK && p->forcing != TSLB_REF_FORCING_GUO) return -1;
   tslb_ref_ctx *c = new (std::nothrow) tslb_ref_ctx();
   if (!c) return -2;
   c->p = *p;
@@ -327,12 +416,15 @@ int tslb_ref_create(const tslb_ref_params *p, tslb_ref_ctx **out) {
   c->gamma = p->two_component ? 2.0 / p->interface_width : 0.0;
   c->t = 0;
   c->inited = false;
+  c->guo = p->forcing == TSLB_REF_FORCING_GUO;
   try {
     const size_t N = c->N;
     c->fpost.assign(27 * N, 0.0); c->fpost2.assign(27 * N, 0.0);
     c->rho.assign(N, 1.0); c->rho2.assign(N, 1.0);
     c->u.assign(3 * N, 0.0); c->u2.assign(3 * N, 0.0);
     c->pineq.assign(6 * N, 0.0); c->pineq2.assign(6 * N, 0.0);
+    c->Ftot.assign(3 * N, 0.0);
+    c->drho_s.assign(N, 0.0);
     if (p->two_component) {
       c->phi.assign(N, 0.0); c->phi2.assign(N, 0.0);
       c->G.assign(3 * N, 0.0); c->nrm.assign(3 * N, 0.0); c->kappa.assign(N, 0.0);
@@ -372,6 +464,13 @@ int tslb_ref_init_fields(tslb_ref_ctx *c, const double *rho, const double *ux, c
     /* boundary planes from the initial fields themselves, hash step index 0 */
     std::vector<double> r0 = c->rho, u0 = c->u, p0 = c->pineq, ph0 = c->phi;
     c->boundary_planes(r0, u0, p0, ph0, c->rho, c->u, c->pineq, c->phi, c->fpost, 0);
+  }
+  std::fill(c->Ftot.begin(), c->Ftot.end(), 0.0);
+  if (c->guo) {
+    /* the given velocity is the stored (bare) one; F(0) from phi(0) enters the first collision */
+    for (size_t i = 0; i < N; ++i) c->drho_s[i] = c->rho[i] - 1.0;
+    c->compute_force();
+    c->collide_all_guo();
   }
   c->inited = true;
   return 0;
@@ -443,6 +542,25 @@ int tslb_ref_phase_geometry(tslb_ref_ctx *c, double *G, double *n, double *kappa
   if (F)
     for (int a = 0; a < 3; ++a)
       for (size_t i = 0; i < N; ++i) F[a * N + i] = c->p.sigma * c->kappa[i] * c->G[a * N + i];
+  return 0;
+}
+
+int tslb_ref_set_extra_force(tslb_ref_ctx *c, const double *Fext) {
+  if (!c) return -1;
+  if (!Fext) { c->Fext.clear(); return 0; }
+  c->Fext.assign(Fext, Fext + 3 * c->N);
+  return 0;
+}
+
+int tslb_ref_get_physical_velocity(tslb_ref_ctx *c, double *ux, double *uy, double *uz) {
+  if (!c) return -1;
+  if (!c->inited) return -4;
+  const size_t N = c->N;
+  double *out[3] = {ux, uy, uz};
+  const double sgn = c->guo ? 0.5 : -0.5;
+  for (int a = 0; a < 3; ++a)
+    if (out[a])
+      for (size_t i = 0; i < N; ++i) out[a][i] = c->u[a * N + i] + sgn * c->Ftot[a * N + i] / c->rho[i];
   return 0;
 }
 

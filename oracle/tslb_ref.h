@@ -21,6 +21,14 @@ extern "C" {
 typedef struct tslb_ref_ctx tslb_ref_ctx;
 
 enum { TSLB_REF_BC_PERIODIC = 0, TSLB_REF_BC_JET_INFLOW = 1, TSLB_REF_BC_OUTFLOW = 2 };
+/* How the force F = sigma kappa grad(phi) (eq. 20) enters the flow solver.  The paper
+ * does not say; both readings are listed in DESIGN.md §3.
+ *   KICK (A9, the default): velocity kick u' = u_b + F/rho' after streaming, F from the OLD phi.
+ *   GUO  (A18): time-centred forcing of Guo, Zheng & Shi, Phys. Rev. E 65 (2002)
+ *        046308: collision velocity u = (m + F/2)/rho, source populations (1 - omega/2) S_i with
+ *        S_i = w_i [ (c_i - u).F / c_s^2 + (c_i.u)(c_i.F) / c_s^4 ],  F evaluated at the time level
+ *        of the populations being collided.  Stored velocity: the bare u_b = m/rho.              */
+enum { TSLB_REF_FORCING_KICK = 0, TSLB_REF_FORCING_GUO = 1 };
 
 typedef struct {
   int nx, ny, nz;          /* grid; x and y always periodic                                 */
@@ -32,6 +40,7 @@ typedef struct {
   int bc_zlo, bc_zhi;      /* PERIODIC/PERIODIC or JET_INFLOW/OUTFLOW                       */
   double jet_diameter, jet_velocity, jet_perturbation;
   unsigned long long seed; /* inflow perturbation seed (reading A12)                        */
+  int forcing;             /* TSLB_REF_FORCING_KICK | TSLB_REF_FORCING_GUO                  */
 } tslb_ref_params;
 
 /* All return 0 on success, negative on error. */
@@ -55,6 +64,14 @@ void tslb_ref_fneq(const double pineq[6], const double u[3], int order, double o
 int tslb_ref_get_populations(tslb_ref_ctx *c, double *fpost);
 /* phase geometry of the CURRENT phi (eqs. 20-21 as read in A6/A7): G[3N], n[3N], kappa[N], F[3N] */
 int tslb_ref_phase_geometry(tslb_ref_ctx *c, double *G, double *n, double *kappa, double *F);
+/* Pin-only probe: a static force density Fext (3N doubles, component-major; NULL clears it) that
+ * is ADDED to sigma kappa grad(phi) at every interior node (also when !two_component).  The method
+ * has no such term; it lets the forcing be pinned on flows with a closed form (uniform
+ * acceleration, Kolmogorov flow).  Call before tslb_ref_init_fields. */
+int tslb_ref_set_extra_force(tslb_ref_ctx *c, const double *Fext);
+/* Time-centred physical velocity of the CURRENT state: KICK: u' - F/(2 rho) with the F that made
+ * the last kick (0 before the first step); GUO: u_b + F/(2 rho) with F of the current phi. */
+int tslb_ref_get_physical_velocity(tslb_ref_ctx *c, double *ux, double *uy, double *uz);
 /* inflow perturbation xi in (-1,1) (reading A12) */
 double tslb_ref_xi(unsigned long long seed, int x, int y, int nx, int ny, long long step);
 /* number of OpenMP threads the step loop uses */
