@@ -57,6 +57,20 @@ enum {
                                when the grid is not supported)                                 */
 };
 
+/* How the surface-tension force F = sigma kappa grad(phi) (eq. 20) enters the flow
+ * solver.  The paper does not say; both readings are listed in DESIGN.md §3.
+ *   TSLB_FORCING_KICK (A9, default): after streaming, u' = u_b + F/rho' with F from the OLD phi;
+ *     the collision is built on u'.  Stored velocity: u'.  All kernels.
+ *   TSLB_FORCING_GUO (A18): time-centred forcing of Guo, Zheng & Shi, Phys. Rev. E
+ *     65 (2002) 046308.  At every source node the collision is built on u = u_b + F/(2 rho) with
+ *     the F of the same time level and carries the source populations (1 - omega/2) S_i,
+ *     S_i = w_i [(c_i - u).F/c_s^2 + (c_i.u)(c_i.F)/c_s^4]; phi is advected with u.  Stored
+ *     velocity: the bare u_b = m/rho (so tslb_init_fields takes u_b and tslb_get_moments returns
+ *     it).  F on a source node needs phi three nodes away, beyond the 2-node phi halo of the tiled
+ *     kernel: this reading runs on TSLB_KERNEL_GENERIC only (F in three scratch arrays), needs
+ *     two_component, and does not take TSLB_BC_HALO faces.                                      */
+enum { TSLB_FORCING_KICK = 0, TSLB_FORCING_GUO = 1 };
+
 typedef struct {
   int nx, ny, nz;          /* grid.  All > 0; nz >= 4 if z is not periodic */
   int precision;           /* TSLB_F32 | TSLB_F64: element type of every field pointer and
@@ -80,6 +94,7 @@ typedef struct {
   void *workspace;         /* optional caller-owned DEVICE memory, 256-byte aligned (e.g. a
                               torch tensor); NULL -> the library allocates with cudaMalloc     */
   size_t workspace_bytes;  /* size of `workspace`; must be >= tslb_workspace_bytes()           */
+  int forcing;             /* TSLB_FORCING_KICK | TSLB_FORCING_GUO                             */
 } tslb_params;
 
 /* Device bytes the context needs: 2 x (10 moment arrays [+ phi]) in the padded internal layout
@@ -102,11 +117,20 @@ int tslb_init_fields(tslb_ctx *c, const void *rho, const void *ux, const void *u
  * the context's stream.  TSLB_ESTATE before tslb_init_fields.                                   */
 int tslb_step(tslb_ctx *c, int nsteps);
 
-/* Copy out the stored state: rho, the stored (post-kick) velocity u' (the time-centred physical
- * velocity is u' - F/(2 rho), reading A9), Pi^neq (NOT the full Pi; reading A2) and phi.  Any
+/* Copy out the stored state: rho, the stored velocity (KICK: the post-kick u'; GUO: the bare u_b;
+ * see tslb_get_physical_velocity), Pi^neq (NOT the full Pi; reading A2; relative to u_b) and phi.  Any
  * pointer (and any entry of pineq, or pineq itself) may be NULL.  Synchronises the stream.      */
 int tslb_get_moments(tslb_ctx *c, void *rho, void *ux, void *uy, void *uz, void *const pineq[6],
                      void *phi, int pointers_on_device);
+
+/* The time-centred ("physical") velocity of the current state, (m_pre + m_post)/(2 rho): the mean of
+ * the momentum before and after the forced collision.  KICK: u' - F/(2 rho) with the F that made
+ * the last kick (from phi of the previous step, still held in the other buffer; F = 0 before the
+ * first step); GUO: u_b + F/(2 rho) with F of the current phi.  F = 0 on inflow/outflow planes and
+ * when !two_component.  Runs the phase-geometry kernels of the generic path into three scratch
+ * arrays (allocated on first use for a tiled context).  Any pointer may be NULL.  Synchronises the
+ * stream.  Not available on a z-slab (TSLB_EINVAL).                                              */
+int tslb_get_physical_velocity(tslb_ctx *c, void *ux, void *uy, void *uz, int pointers_on_device);
 
 /* ---- z-slabs: one domain split along z over several contexts / GPUs (the paper's
  * stated next step).  Every node update reads only time-t values within one

@@ -87,6 +87,12 @@ Validated validate(const tslb_params *p) {
   }
   if ((v.jet_lo || v.out_hi) && !(p->jet_diameter >= 0.0)) return fail("jet_diameter must be >= 0");
   if (p->kernel < TSLB_KERNEL_AUTO || p->kernel > TSLB_KERNEL_TILED) return fail("unknown kernel selector");
+  if (p->forcing != TSLB_FORCING_KICK && p->forcing != TSLB_FORCING_GUO) return fail("unknown forcing selector");
+  const bool guo = p->forcing == TSLB_FORCING_GUO;
+  if (guo && !p->two_component) return fail("TSLB_FORCING_GUO needs two_component (the force comes from phi)");
+  if (guo && v.slab) return fail("TSLB_FORCING_GUO does not take TSLB_BC_HALO faces");
+  if (guo && p->kernel == TSLB_KERNEL_TILED)
+    return fail("TSLB_FORCING_GUO runs on TSLB_KERNEL_GENERIC only (the force on a source node needs a 3-node phi halo)");
   v.zper = zper;
   v.esize = p->precision == TSLB_F32 ? 4 : 8;
   v.nfields = p->two_component ? 11 : 10;
@@ -94,10 +100,12 @@ Validated validate(const tslb_params *p) {
   const bool tiled_ok = tiled_supported(p->precision, p->nx, p->ny, p->nz);
   if (p->kernel == TSLB_KERNEL_TILED && !tiled_ok)
     return fail("TSLB_KERNEL_TILED needs nx >= 32, ny >= 8 and nx a multiple of 4 (fp32) or 2 (fp64)");
-  v.kernel = (p->kernel == TSLB_KERNEL_GENERIC || !tiled_ok) ? TSLB_KERNEL_GENERIC : TSLB_KERNEL_TILED;
-  // 2 buffers x nfields arrays, + 3 scratch arrays for the generic two-component path
+  v.kernel = (p->kernel == TSLB_KERNEL_GENERIC || !tiled_ok || guo) ? TSLB_KERNEL_GENERIC : TSLB_KERNEL_TILED;
+  // 2 buffers x nfields arrays, + 3 scratch arrays (n) for the generic two-component path,
+  // + 3 more (F) for TSLB_FORCING_GUO
   size_t narr = 2 * (size_t)v.nfields;
   if (v.kernel == TSLB_KERNEL_GENERIC && p->two_component) narr += 3;
+  if (guo) narr += 3;
   v.bytes = narr * round_up((size_t)v.L.field * v.esize, 256);
   v.ok = true;
   return v;
@@ -113,6 +121,8 @@ struct tslb_ctx {
   bool own_ws = false;
   void *fields[2][NF_MAX] = {};
   void *nrm[3] = {};
+  void *frc[3] = {};           // TSLB_FORCING_GUO: scratch force arrays
+  void *nrm_own = nullptr;     // scratch n allocated by tslb_get_physical_velocity on a tiled context
   void *nb_fields[2][2][NF_MAX] = {};   // [side][buffer][field]: neighbour slabs' arrays (peer pointers)
   int nb_nz[2] = {0, 0};
   bool nb_on[2] = {false, false};
@@ -161,7 +171,7 @@ StepParams<T> make_step_params(tslb_ctx *c, int src, int dst) {
     P.in.f[k] = (T *)c->fields[src][k];
     P.out.f[k] = (T *)c->fields[dst][k];
   }
-  for (int k = 0; k < 3; ++k) P.nrm[k] = (T *)c->nrm[k];
+  for (int k = 0; k < 3; ++k) { P.nrm[k] = (T *)c->nrm[k]; P.frc[k] = (T *)c->frc[k]; }
   P.omc = (T)(1.0 - c->p.omega);
   P.sigma = (T)(c->p.two_component ? c->p.sigma : 0.0);
   P.gamma = (T)(c->p.two_component ? 2.0 / c->p.interface_width : 0.0);
@@ -191,7 +201,13 @@ int launch_generic(tslb_ctx *c, const StepParams<T> &P) {
   }
   dim3 b(32, 4), g((L.nx + 31) / 32, (L.ny + 3) / 4, L.nz);
   const int o3 = c->p.hermite_order >= 3;
-  if (two) {
+  if (c->p.forcing == TSLB_FORCING_GUO) {
+    dim3 bf(32, 8), gf((L.nx + 31) / 32, (L.ny + 7) / 8, L.nz);
+    force_kernel<T><<<gf, bf, 0, c->stream>>>(P);
+    c->launches++;
+    if (o3) generic_step_kernel<T, 3, true, true><<<g, b, 0, c->stream>>>(P);
+    else generic_step_kernel<T, 2, true, true><<<g, b, 0, c->stream>>>(P);
+  } else if (two) {
     if (o3) generic_step_kernel<T, 3, true><<<g, b, 0, c->stream>>>(P);
     else generic_step_kernel<T, 2, true><<<g, b, 0, c->stream>>>(P);
   } else {
@@ -236,6 +252,54 @@ int step_typed(tslb_ctx *c, int nsteps) {
       c->stat_n++;
     }
   }
+  return TSLB_OK;
+}
+
+// tslb_get_physical_velocity: n of the phi that made the force into scratch, then one kernel
+template <typename T>
+int physvel_typed(tslb_ctx *c, void *const dst[3], int on_device) {
+  const Layout &L = c->v.L;
+  const size_t N = (size_t)L.nx * L.ny * L.nz;
+  const bool guo = c->p.forcing == TSLB_FORCING_GUO;
+  const bool use_force = c->p.two_component && (guo || c->t >= 1);
+  // GUO: F of the current phi; KICK: F of the previous step's phi, still in the other buffer
+  const int src = guo ? c->cur : c->cur ^ 1;
+  StepParams<T> P = make_step_params<T>(c, src, src);
+  for (int side = 0; side < 2; ++side)
+    for (int k = 0; k < NF_MAX; ++k) P.nb[side].f[k] = nullptr;
+  if (use_force) {
+    if (!c->nrm[0]) {
+      const size_t fb = round_up((size_t)L.field * sizeof(T), 256);
+      if (!c->nrm_own) {
+        cudaError_t e = cudaMalloc(&c->nrm_own, 3 * fb);
+        if (e != cudaSuccess) return c->fail(TSLB_ENOMEM, "cudaMalloc(scratch normals): %s", cudaGetErrorString(e));
+      }
+      for (int k = 0; k < 3; ++k) P.nrm[k] = (T *)((char *)c->nrm_own + k * fb);
+    }
+    dim3 b(32, 8), g((L.nx + 31) / 32, (L.ny + 7) / 8, L.nz);
+    phase_normals_kernel<T><<<g, b, 0, c->stream>>>(P);
+    CK(cudaGetLastError());
+  }
+  FieldSet<T> vel;
+  for (int k = 0; k < NF_MAX; ++k) vel.f[k] = (T *)c->fields[c->cur][k];
+  // host destinations: the three components go through scratch device memory of their own
+  T *dev[3] = {nullptr, nullptr, nullptr};
+  T *tmp = nullptr;
+  if (!on_device) {
+    CK(cudaMalloc((void **)&tmp, 3 * N * sizeof(T)));
+    for (int a = 0; a < 3; ++a) dev[a] = dst[a] ? tmp + a * N : nullptr;
+  } else {
+    for (int a = 0; a < 3; ++a) dev[a] = (T *)dst[a];
+  }
+  dim3 b(32, 8), g((L.nx + 31) / 32, (L.ny + 7) / 8, L.nz);
+  physical_velocity_kernel<T><<<g, b, 0, c->stream>>>(P, vel, guo ? T(0.5) : T(-0.5), use_force ? 1 : 0, dev[0], dev[1], dev[2]);
+  cudaError_t e = cudaGetLastError();
+  if (e == cudaSuccess && !on_device)
+    for (int a = 0; a < 3 && e == cudaSuccess; ++a)
+      if (dst[a]) e = cudaMemcpyAsync(dst[a], dev[a], N * sizeof(T), cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  if (tmp) cudaFree(tmp);
+  if (e != cudaSuccess) return c->cuda_fail(e, "tslb_get_physical_velocity");
   return TSLB_OK;
 }
 
@@ -365,6 +429,8 @@ int tslb_create(const tslb_params *p, tslb_ctx **out) {
   carve_fields(c->ws, v.L, v.esize, v.nfields, c->fields, &off);
   if (v.kernel == TSLB_KERNEL_GENERIC && p->two_component)
     for (int k = 0; k < 3; ++k) { c->nrm[k] = base + off + (size_t)v.L.gz * v.L.plane * v.esize; off += fb; }
+  if (p->forcing == TSLB_FORCING_GUO)
+    for (int k = 0; k < 3; ++k) { c->frc[k] = base + off; off += fb; }
   if (v.kernel == TSLB_KERNEL_TILED) {
     std::string why;
     if (!tiled_plan_create(c->tiled, p->precision, v.L, c->fields, v.nfields, p->device, why)) {
@@ -380,7 +446,7 @@ int tslb_create(const tslb_params *p, tslb_ctx **out) {
     }
     c->kname = c->use_ws ? "tiled-ws" + c->tiled.name.substr(5) : c->tiled.name;
   } else {
-    c->kname = "generic";
+    c->kname = p->forcing == TSLB_FORCING_GUO ? "generic-guo" : "generic";
   }
   *out = c;
   return TSLB_OK;
@@ -436,6 +502,16 @@ int tslb_get_moments(tslb_ctx *c, void *rho, void *ux, void *uy, void *uz, void 
     for (int k = 0; k < 6; ++k) dst[F_PXX + k] = pineq[k];
   return c->p.precision == TSLB_F32 ? get_typed<float>(c, dst, pointers_on_device)
                                     : get_typed<double>(c, dst, pointers_on_device);
+}
+
+int tslb_get_physical_velocity(tslb_ctx *c, void *ux, void *uy, void *uz, int pointers_on_device) {
+  if (!c) return TSLB_EINVAL;
+  if (!c->inited) return c->fail(TSLB_ESTATE, "tslb_get_physical_velocity before tslb_init_fields");
+  if (c->v.slab) return c->fail(TSLB_EINVAL, "tslb_get_physical_velocity is not available on a z-slab");
+  CK(cudaSetDevice(c->p.device));
+  void *dst[3] = {ux, uy, uz};
+  return c->p.precision == TSLB_F32 ? physvel_typed<float>(c, dst, pointers_on_device)
+                                    : physvel_typed<double>(c, dst, pointers_on_device);
 }
 
 void *tslb_workspace_ptr(const tslb_ctx *c) { return c ? c->ws : nullptr; }
@@ -576,6 +652,7 @@ int tslb_destroy(tslb_ctx *c) {
     if (c->nb_ipc[side]) cudaIpcCloseMemHandle(c->nb_ipc[side]);
   if (c->stage) cudaFree(c->stage);
   if (c->stat) cudaFree(c->stat);
+  if (c->nrm_own) cudaFree(c->nrm_own);
   if (c->own_ws && c->ws) cudaFree(c->ws);
   delete c;
   return TSLB_OK;

@@ -47,6 +47,7 @@ struct StepParams {
   Layout L;
   FieldSet<T> in, out;   // time t (read only) and time t+1 (written)
   T *nrm[3];             // generic path only: scratch n = grad(phi)/(|grad(phi)|+eps), dense padded
+  T *frc[3];             // TSLB_FORCING_GUO only: scratch F = sigma kappa grad(phi) of the time-t phi
   T omc;                 // 1 - omega                               (eq. 5)
   T sigma;               // surface tension                         (eq. 20)
   T gamma;               // anti-diffusion 2/W                      (eq. 24, A8)

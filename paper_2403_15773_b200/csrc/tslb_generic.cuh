@@ -44,6 +44,32 @@ __device__ __forceinline__ void grad_phi(const T *__restrict__ phi, const StepPa
   G[0] = gx; G[1] = gy; G[2] = gz;
 }
 
+// kappa = -(1/c_s^2) sum_i w_i c_i . n(x + c_i) from the scratch normals   (eq. 21, A6)
+template <typename T>
+__device__ __forceinline__ T kappa_at(const StepParams<T> &P, int x, int y, int z) {
+  const Layout &L = P.L;
+  T div = T(0);
+#pragma unroll
+  for (int dz = -1; dz <= 1; ++dz) {
+    const int zz = zsrc(P, z + dz);
+#pragma unroll
+    for (int dy = -1; dy <= 1; ++dy) {
+      const int yy = wrapi(y + dy, L.ny);
+#pragma unroll
+      for (int dx = -1; dx <= 1; ++dx) {
+        if (dx == 0 && dy == 0 && dz == 0) continue;
+        const int xx = wrapi(x + dx, L.nx);
+        const long long j = L.idx(xx, yy, zz);
+        const T w = w1d<T>(dx) * w1d<T>(dy) * w1d<T>(dz) * T(3);
+        if (dx != 0) div += (w * T(dx)) * P.nrm[0][j];
+        if (dy != 0) div += (w * T(dy)) * P.nrm[1][j];
+        if (dz != 0) div += (w * T(dz)) * P.nrm[2][j];
+      }
+    }
+  }
+  return -div;
+}
+
 template <typename T>
 __global__ void __launch_bounds__(256) phase_normals_kernel(const __grid_constant__ StepParams<T> P) {
   const Layout &L = P.L;
@@ -86,7 +112,50 @@ __device__ __forceinline__ void boundary_node(const StepParams<T> &P, const Fiel
   }
 }
 
-template <typename T, int ORDER, bool TWO>
+// F = sigma kappa G of the time-t phi into the scratch arrays frc (TSLB_FORCING_GUO), zero on the
+// inflow/outflow planes (their moments are imposed, O9).  Needs phase_normals_kernel first.
+template <typename T>
+__global__ void __launch_bounds__(256) force_kernel(const __grid_constant__ StepParams<T> P) {
+  const Layout &L = P.L;
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  const int y = blockIdx.y * blockDim.y + threadIdx.y;
+  const int z = blockIdx.z;
+  if (x >= L.nx || y >= L.ny) return;
+  T s = T(0), G[3] = {T(0), T(0), T(0)};
+  if (!((P.jet_lo && z == 0) || (P.out_hi && z == L.nz - 1))) {
+    grad_phi<T>(P.in.f[F_PHI], P, x, y, z, G);
+    s = P.sigma * kappa_at<T>(P, x, y, z);
+  }
+  const long long i = L.idx(x, y, z);
+  P.frc[0][i] = s * G[0];
+  P.frc[1][i] = s * G[1];
+  P.frc[2][i] = s * G[2];
+}
+
+// Time-centred velocity (include/tslb.h tslb_get_physical_velocity) into dense arrays: the stored
+// velocity of `vel` plus sgn * F / rho, F = sigma kappa G of the phi in P.in (needs
+// phase_normals_kernel on the same P first); F = 0 on inflow/outflow planes and when !use_force.
+template <typename T>
+__global__ void __launch_bounds__(256) physical_velocity_kernel(const __grid_constant__ StepParams<T> P, FieldSet<T> vel,
+                                                                T sgn, int use_force, T *dx_, T *dy_, T *dz_) {
+  const Layout &L = P.L;
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  const int y = blockIdx.y * blockDim.y + threadIdx.y;
+  const int z = blockIdx.z;
+  if (x >= L.nx || y >= L.ny) return;
+  T s = T(0), G[3] = {T(0), T(0), T(0)};
+  const long long i = L.idx(x, y, z);
+  if (use_force && !((P.jet_lo && z == 0) || (P.out_hi && z == L.nz - 1))) {
+    grad_phi<T>(P.in.f[F_PHI], P, x, y, z, G);
+    s = sgn * P.sigma * kappa_at<T>(P, x, y, z) / (T(1) + vel.f[F_DRHO][i]);
+  }
+  const long long o = (long long)x + (long long)L.nx * (y + (long long)L.ny * z);
+  if (dx_) dx_[o] = vel.f[F_UX][i] + s * G[0];
+  if (dy_) dy_[o] = vel.f[F_UY][i] + s * G[1];
+  if (dz_) dz_[o] = vel.f[F_UZ][i] + s * G[2];
+}
+
+template <typename T, int ORDER, bool TWO, bool GUO = false>
 __global__ void __launch_bounds__(128) generic_step_kernel(const __grid_constant__ StepParams<T> P) {
   const Layout &L = P.L;
   const int x = blockIdx.x * blockDim.x + threadIdx.x;
@@ -120,9 +189,15 @@ __global__ void __launch_bounds__(128) generic_step_kernel(const __grid_constant
         const int xx = wrapi(x - cx, L.nx);
         const long long j = L.idx(xx, yy, zz);
         T Kt[NK];
-        post_collision_coeffs<ORDER, T>(P.in.f[F_DRHO][j], P.in.f[F_UX][j], P.in.f[F_UY][j], P.in.f[F_UZ][j],
-                                        P.in.f[F_PXX][j], P.in.f[F_PYY][j], P.in.f[F_PZZ][j], P.in.f[F_PXY][j],
-                                        P.in.f[F_PXZ][j], P.in.f[F_PYZ][j], P.omc, Kt);
+        if (GUO)
+          post_collision_coeffs_guo<ORDER, T>(P.in.f[F_DRHO][j], P.in.f[F_UX][j], P.in.f[F_UY][j], P.in.f[F_UZ][j],
+                                              P.in.f[F_PXX][j], P.in.f[F_PYY][j], P.in.f[F_PZZ][j], P.in.f[F_PXY][j],
+                                              P.in.f[F_PXZ][j], P.in.f[F_PYZ][j], P.frc[0][j], P.frc[1][j], P.frc[2][j],
+                                              P.omc, Kt);
+        else
+          post_collision_coeffs<ORDER, T>(P.in.f[F_DRHO][j], P.in.f[F_UX][j], P.in.f[F_UY][j], P.in.f[F_UZ][j],
+                                          P.in.f[F_PXX][j], P.in.f[F_PYY][j], P.in.f[F_PZZ][j], P.in.f[F_PXY][j],
+                                          P.in.f[F_PXZ][j], P.in.f[F_PYZ][j], P.omc, Kt);
         const T x1 = h1d<T>(1, cx), x2 = h1d<T>(2, cx);
         const T y1 = h1d<T>(1, cy), y2 = h1d<T>(2, cy);
         const T z1 = h1d<T>(1, cz), z2 = h1d<T>(2, cz);
@@ -144,32 +219,15 @@ __global__ void __launch_bounds__(128) generic_step_kernel(const __grid_constant
 
   T phin = T(0);
   if (TWO) {
-    // a5: G at the node from the OLD phi; kappa = -(1/c_s^2) sum_i w_i c_i . n(x + c_i)
-    T G[3];
-    grad_phi<T>(P.in.f[F_PHI], P, x, y, z, G);
-    T div = T(0);
-#pragma unroll
-    for (int dz = -1; dz <= 1; ++dz) {
-      const int zz = zsrc(P, z + dz);
-#pragma unroll
-      for (int dy = -1; dy <= 1; ++dy) {
-        const int yy = wrapi(y + dy, L.ny);
-#pragma unroll
-        for (int dx = -1; dx <= 1; ++dx) {
-          if (dx == 0 && dy == 0 && dz == 0) continue;
-          const int xx = wrapi(x + dx, L.nx);
-          const long long j = L.idx(xx, yy, zz);
-          const T w = w1d<T>(dx) * w1d<T>(dy) * w1d<T>(dz) * T(3);
-          if (dx != 0) div += (w * T(dx)) * P.nrm[0][j];
-          if (dy != 0) div += (w * T(dy)) * P.nrm[1][j];
-          if (dz != 0) div += (w * T(dz)) * P.nrm[2][j];
-        }
-      }
+    if (!GUO) {
+      // a5: G at the node from the OLD phi; kappa = -(1/c_s^2) sum_i w_i c_i . n(x + c_i)
+      T G[3];
+      grad_phi<T>(P.in.f[F_PHI], P, x, y, z, G);
+      const T kappa = kappa_at<T>(P, x, y, z);
+      // a6: kick u' = u_b + F / rho', F = sigma kappa G   (A9)
+      const T s = P.sigma * kappa / (T(1) + drho);
+      ub[0] += s * G[0]; ub[1] += s * G[1]; ub[2] += s * G[2];
     }
-    const T kappa = -div;
-    // a6: kick u' = u_b + F / rho', F = sigma kappa G   (A9)
-    const T s = P.sigma * kappa / (T(1) + drho);
-    ub[0] += s * G[0]; ub[1] += s * G[1]; ub[2] += s * G[2];
     // a7: phi'(x) = sum_{i in D3Q7} w_i [ phi (1 + c_i.u / c_sg^2) + gamma phi (1-phi) c_i.n ](x - c_i)
     const T *phi = P.in.f[F_PHI];
     const T pc = phi[i0];
@@ -185,7 +243,9 @@ __global__ void __launch_bounds__(128) generic_step_kernel(const __grid_constant
 #pragma unroll
     for (int q = 0; q < 6; ++q) {
       const T p = phi[jn[q]];
-      const T uc = P.in.f[F_UX + comp[q]][jn[q]];
+      T uc = P.in.f[F_UX + comp[q]][jn[q]];
+      // A18: phi is advected with the time-centred velocity u_b + F/(2 rho) of the source node
+      if (GUO) uc += P.frc[comp[q]][jn[q]] / (T(2) * (T(1) + P.in.f[F_DRHO][jn[q]]));
       const T nc = P.nrm[comp[q]][jn[q]];
       acc += T(0.125) * (p * (T(1) + sgn[q] * T(4) * uc) + P.gamma * p * (T(1) - p) * (sgn[q] * nc));
     }

@@ -65,6 +65,36 @@ __device__ __forceinline__ void post_collision_coeffs(V drho, V ux, V uy, V uz, 
   }
 }
 
+// Reading A18 (include/tslb.h TSLB_FORCING_GUO; Guo, Zheng & Shi 2002): the same coefficients for a
+// node whose stored moments are the BARE ones (u_b = m/rho, Pi_b^neq relative to u_b) and which
+// carries the force F.  Collision velocity u = u_b + F/(2 rho); non-equilibrium stress relative to
+// u: Pi^neq = Pi_b^neq + rho (u_b u_b - u u); and on top of f^eq(u) + (1-omega) f^neq(Pi^neq, u):
+//   first order   rho u + (1-omega)(m - rho u) + (1-omega/2) F  =  rho u + F/2        (= m + F)
+//   second order  + (1-omega/2)(u F + F u)                          (moments of the source S_i)
+// The source has no third-order part, so K_210.. K_111 are those of the unforced formula.
+template <int ORDER, typename V>
+__device__ __forceinline__ void post_collision_coeffs_guo(V drho, V ubx, V uby, V ubz, V pxx, V pyy, V pzz,
+                                                          V pxy, V pxz, V pyz, V fx, V fy, V fz, V omc, V *Kt) {
+  const V rho = drho + V(1);
+  const V h = V(0.5) / rho;
+  const V ux = ubx + fx * h, uy = uby + fy * h, uz = ubz + fz * h;
+  post_collision_coeffs<ORDER, V>(drho, ux, uy, uz,
+                                  pxx + (rho * ubx * ubx - rho * ux * ux), pyy + (rho * uby * uby - rho * uy * uy),
+                                  pzz + (rho * ubz * ubz - rho * uz * uz), pxy + (rho * ubx * uby - rho * ux * uy),
+                                  pxz + (rho * ubx * ubz - rho * ux * uz), pyz + (rho * uby * ubz - rho * uy * uz),
+                                  omc, Kt);
+  const V s = V(0.5) * (V(1) + omc);   // 1 - omega/2
+  Kt[K100] += V(1.5) * fx;
+  Kt[K010] += V(1.5) * fy;
+  Kt[K001] += V(1.5) * fz;
+  Kt[K200] += V(9) * s * (ux * fx);
+  Kt[K020] += V(9) * s * (uy * fy);
+  Kt[K002] += V(9) * s * (uz * fz);
+  Kt[K110] += V(9) * s * (ux * fy + uy * fx);
+  Kt[K101] += V(9) * s * (ux * fz + uz * fx);
+  Kt[K011] += V(9) * s * (uy * fz + uz * fy);
+}
+
 // Un-normalised Hermite coefficients K_abc (same 17, same order) with explicit FMAs, for the
 // tiled kernel where V is a packed pair; the 1/norm factors are folded into the 1-D operators.
 template <int ORDER, typename V>

@@ -16,9 +16,10 @@ OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
 F32, F64 = 0, 1
 BC_PERIODIC, BC_JET_INFLOW, BC_OUTFLOW, BC_HALO = 0, 1, 2, 3
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED = 0, 1, 2
+FORCING_KICK, FORCING_GUO = 0, 1
 
 EXPORTS = ["tslb_workspace_bytes", "tslb_create", "tslb_init_fields", "tslb_step",
-           "tslb_get_moments", "tslb_step_count", "tslb_kernel_name", "tslb_launch_count",
+           "tslb_get_moments", "tslb_get_physical_velocity", "tslb_step_count", "tslb_kernel_name", "tslb_launch_count",
            "tslb_debug_xi", "tslb_destroy", "tslb_last_error", "tslb_workspace_ptr",
            "tslb_attach_neighbor", "tslb_ipc_get_handle", "tslb_attach_neighbor_ipc", "tslb_halo_push",
            "tslb_stats_begin", "tslb_stats_get", "tslb_stats_end"]
@@ -39,6 +40,7 @@ class Params(ctypes.Structure):
         ("device", ctypes.c_int), ("kernel", ctypes.c_int),
         ("stream", ctypes.c_void_p), ("workspace", ctypes.c_void_p),
         ("workspace_bytes", ctypes.c_size_t),
+        ("forcing", ctypes.c_int),
     ]
 
 
@@ -66,6 +68,7 @@ def lib():
         L.tslb_init_fields.argtypes = [vp, vp, vp, vp, vp, vp, ctypes.POINTER(vp), ctypes.c_int]
         L.tslb_step.argtypes = [vp, ctypes.c_int]
         L.tslb_get_moments.argtypes = [vp, vp, vp, vp, vp, ctypes.POINTER(vp), vp, ctypes.c_int]
+        L.tslb_get_physical_velocity.argtypes = [vp, vp, vp, vp, ctypes.c_int]
         L.tslb_step_count.argtypes = [vp]
         L.tslb_step_count.restype = ctypes.c_longlong
         L.tslb_kernel_name.argtypes = [vp]
@@ -92,13 +95,13 @@ def lib():
 def make_params(nx, ny, nz, omega, precision=F32, two_component=False, hermite_order=3, sigma=0.0,
                 interface_width=4.0, jet=False, jet_diameter=0.0, jet_velocity=0.0,
                 jet_perturbation=0.0, seed=0, device=0, kernel=KERNEL_AUTO, stream=None,
-                workspace=None, workspace_bytes=0, bc_zlo=None, bc_zhi=None):
+                workspace=None, workspace_bytes=0, bc_zlo=None, bc_zhi=None, forcing=FORCING_KICK):
     """`jet` sets JET_INFLOW/OUTFLOW; bc_zlo / bc_zhi override one face (BC_HALO for a z-slab)."""
     lo = (BC_JET_INFLOW if jet else BC_PERIODIC) if bc_zlo is None else bc_zlo
     hi = (BC_OUTFLOW if jet else BC_PERIODIC) if bc_zhi is None else bc_zhi
     return Params(nx, ny, nz, precision, int(bool(two_component)), hermite_order, omega, sigma,
                   interface_width, lo, hi, jet_diameter, jet_velocity, jet_perturbation,
-                  seed, device, kernel, stream, workspace, workspace_bytes)
+                  seed, device, kernel, stream, workspace, workspace_bytes, int(forcing))
 
 
 def workspace_bytes(**kw):
@@ -221,6 +224,18 @@ class Tslb:
             out["pineq"] = torch.stack(comps) if device else np.stack(comps)
         out["phi"] = phi
         return out
+
+    def get_physical_velocity(self, device=False):
+        """-> (3, nz, ny, nx) numpy array (or torch CUDA tensor): the time-centred velocity."""
+        torch = self._torch
+        if device:
+            u = torch.empty((3,) + self.shape, dtype=self.torch_dtype, device=self.device)
+            ptrs = [u[a].data_ptr() for a in range(3)]
+        else:
+            u = np.empty((3,) + self.shape, dtype=self.np_dtype)
+            ptrs = [u[a].ctypes.data for a in range(3)]
+        self._check(lib().tslb_get_physical_velocity(self._h, ptrs[0], ptrs[1], ptrs[2], int(device)))
+        return u
 
     # -- z-slabs (include/tslb.h "z-slabs")
     @property

@@ -57,6 +57,11 @@ def test_workspace_bytes(lib):
     assert ws(nx=32, ny=32, nz=32, omega=1.8, precision=tslb.F64) == 20 * field_bytes(32, 32, 32, 8)
     # generic two-component path carries 3 scratch arrays (n)
     assert ws(nx=20, ny=12, nz=10, omega=1.0, two_component=True) == 25 * field_bytes(20, 12, 10, 4)
+    # TSLB_FORCING_GUO: generic path + 3 more scratch arrays (F); no tiled kernel, needs two_component
+    assert ws(nx=64, ny=64, nz=64, omega=1.0, two_component=True, forcing=tslb.FORCING_GUO) == 28 * field_bytes(64, 64, 64, 4)
+    assert ws(nx=64, ny=64, nz=64, omega=1.0, two_component=True, forcing=tslb.FORCING_GUO, kernel=tslb.KERNEL_TILED) == 0
+    assert ws(nx=64, ny=64, nz=64, omega=1.0, forcing=tslb.FORCING_GUO) == 0
+    assert ws(nx=64, ny=64, nz=64, omega=1.0, two_component=True, forcing=2) == 0
     # invalid parameters -> 0
     assert ws(nx=0, ny=4, nz=4, omega=1.0) == 0
     assert ws(nx=4, ny=4, nz=4, omega=2.0) == 0
