@@ -48,6 +48,10 @@ def parse():
                     help="N > 1: independent replicas (default, weak scaling) or ONE domain split into z-slabs "
                          "(strong scaling, halo push fused into the step kernel; DESIGN.md §8)")
     ap.add_argument("--slabs", type=int, default=0, help="with --decomp slabs on one GPU: number of in-process slabs")
+    ap.add_argument("--forcing", default="kick", choices=["kick", "guo"],
+                    help="how the surface-tension force enters (include/tslb.h): the kick of reading A9 (default, all "
+                         "kernels) or the Guo-type forcing of reading A18 (generic kernel only; its cost is a bench line "
+                         "of its own, not the headline)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     return ap.parse_args()
@@ -323,6 +327,8 @@ def main():
         omega = prm["omega"]
         kw = {k: v for k, v in prm.items() if k not in ("nx", "ny", "nz", "omega")}
         state = developed_jet_device(torch, nx, ny, nz, D, prm["jet_velocity"], tdt, dev)
+    if args.forcing == "guo":
+        kw["forcing"] = tslb.FORCING_GUO
     sim = tslb.Tslb(nx, ny, nz, omega, precision=prec, device=local, kernel=kern, **kw)
     sim.init_fields(state["rho"], state["ux"], state["uy"], state["uz"], state["phi"])
     nodes = nx * ny * nz
@@ -425,7 +431,8 @@ def main():
            "config": {"workload": desc, "grid": [nx, ny, nz], "state_bytes_per_gpu": 2 * 11 * nodes * (4 if prec == tslb.F32 else 8),
                       "l2": "state (%.1f GB) far exceeds the 126 MB L2; no flush needed" % (2 * 11 * nodes * 4 / 1e9),
                       "parallelism": "replicas x%d" % world if world > 1 else "single GPU",
-                      "initial_state": "seeded synthetic developed jet (device-generated)", "finite": finite},
+                      "initial_state": "seeded synthetic developed jet (device-generated)", "finite": finite,
+                      "forcing": args.forcing},
            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
            "paper_context": "paper: ~1.5 GLUPS RTX 3090, ~2 GLUPS A100 on 400x400x800 (PAPER.md:283); other hardware, not the target"}
     print(json.dumps(out))
