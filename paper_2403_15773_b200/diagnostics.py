@@ -24,3 +24,25 @@ def radial_profile(avg, z):
     r = np.abs(np.arange(nx) - (nx - 1) / 2.0)
     order = np.argsort(r, kind="stable")
     return r[order], avg[z][order]
+
+
+def linear_fit(x, y):
+    """Least-squares line y = slope * x + intercept -> (slope, intercept, rms residual)."""
+    a = np.vstack([x, np.ones_like(x)]).T
+    (slope, icpt), _, _, _ = np.linalg.lstsq(a, y, rcond=None)
+    r = y - (slope * x + icpt)
+    return float(slope), float(icpt), float(np.sqrt((r ** 2).mean()))
+
+
+def gaussian_exponent(r, q, zeff, lo=0.1, hi=0.95):
+    """K of the best fit q(r)/q_c = exp(-K (r/zeff)^2) (K = 75 for <u_z> at 12 D with
+    zeff = z - z0), least squares on ln(q/q_c) over the points with lo < q/q_c < hi; r sorted
+    ascending (radial_profile), q_c = mean of the two points next to the axis.  None if too few."""
+    qc = q[:2].mean()
+    if not qc > 0:
+        return None
+    ok = (q > lo * qc) & (q < hi * qc)
+    if ok.sum() < 5:
+        return None
+    eta2 = (r[ok] / zeff) ** 2
+    return -float(np.sum(np.log(q[ok] / qc) * eta2) / np.sum(eta2 ** 2))

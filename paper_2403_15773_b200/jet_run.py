@@ -30,6 +30,8 @@ def parse():
     ap.add_argument("--every", type=int, default=10, help="sample the averages every this many steps")
     ap.add_argument("--chunk", type=int, default=2000, help="steps between finiteness checks")
     ap.add_argument("--order", type=int, default=3, help="hermite_order (3: eqs. 16/19, 2: eq. 8)")
+    ap.add_argument("--forcing", default="kick", choices=["kick", "guo"],
+                    help="reading A9 (all kernels) or A18 (Guo-type, generic kernel; include/tslb.h)")
     ap.add_argument("--precision", default="f32")
     ap.add_argument("--perturbation", type=float, default=0.05)
     ap.add_argument("--seed", type=int, default=2024)
@@ -37,11 +39,7 @@ def parse():
     return ap.parse_args()
 
 
-def linear_fit(x, y):
-    a = np.vstack([x, np.ones_like(x)]).T
-    (slope, icpt), res, _, _ = np.linalg.lstsq(a, y, rcond=None)
-    r = y - (slope * x + icpt)
-    return float(slope), float(icpt), float(np.sqrt((r ** 2).mean()))
+linear_fit = diagnostics.linear_fit
 
 
 def main():
@@ -55,13 +53,15 @@ def main():
     prec = tslb.F32 if args.precision == "f32" else tslb.F64
     tdt = torch.float32 if prec == tslb.F32 else torch.float64
     dev = torch.device("cuda", 0)
+    if args.forcing == "guo":
+        kw["forcing"] = tslb.FORCING_GUO
     sim = tslb.Tslb(nx, ny, nz, prm["omega"], precision=prec, hermite_order=args.order, **kw)
     one = torch.ones((nz, ny, nx), dtype=tdt, device=dev)
     zero = torch.zeros((nz, ny, nx), dtype=tdt, device=dev)
     sim.init_fields(one, zero, zero.clone(), zero.clone(), zero.clone())
     del one, zero
     out = {"grid": [nx, ny, nz], "D": D, "U": U, "Re": args.Re, "We": args.We, "omega": prm["omega"],
-           "sigma": prm["sigma"], "hermite_order": args.order, "precision": args.precision,
+           "sigma": prm["sigma"], "hermite_order": args.order, "forcing": args.forcing, "precision": args.precision,
            "kernel": sim.kernel_name, "steps": args.steps, "avg_from": args.avg_from, "every": args.every}
     t0 = time.time()
     done, blew_up = 0, None
@@ -123,18 +123,12 @@ def main():
                 if z12 < nz and s > 0:
                     z0 = -i0 / s * D
                     r, q = diagnostics.radial_profile(st["uz"], z12)
-                    qc = q[:2].mean()
-                    ok = (q > 0.1 * qc) & (q < 0.95 * qc)
-                    if ok.sum() > 4:
-                        eta2 = (r[ok] / (z12 - z0)) ** 2
-                        K = -float(np.sum(np.log(q[ok] / qc) * eta2) / np.sum(eta2 ** 2))
-                        out["gaussian_K_at_12D"] = {"K": K, "paper_K": 75.0, "z0": z0, "points": int(ok.sum())}
+                    K = diagnostics.gaussian_exponent(r, q, z12 - z0)
+                    if K is not None:
+                        out["gaussian_K_at_12D"] = {"K": K, "paper_K": 75.0, "z0": z0}
                     r, q = diagnostics.radial_profile(st["phi"], z12)
-                    qc = q[:2].mean()
-                    ok = (q > 0.1 * qc) & (q < 0.95 * qc)
-                    if qc > 1e-6 and ok.sum() > 4:
-                        eta2 = (r[ok] / (z12 - z0)) ** 2
-                        Kp = -float(np.sum(np.log(q[ok] / qc) * eta2) / np.sum(eta2 ** 2))
+                    Kp = diagnostics.gaussian_exponent(r, q, z12 - z0)
+                    if Kp is not None:
                         out["gaussian_Kint_phi_at_12D"] = {"K": Kp, "paper_K_We2000": 80.0}
     sim.close()
     s = json.dumps(out)
