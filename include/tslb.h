@@ -1,6 +1,6 @@
 /*
  * tslb.h -- C ABI of the B200-native thread-safe lattice Boltzmann (TSLB) two-component time
- * step of arxiv 2403.15773 ("PAPER.md" below = /root/reference/PAPER.md; readings A1..A17 are
+ * step of arxiv 2403.15773 ("PAPER.md" below = /root/reference/PAPER.md; readings A1..A18 are
  * listed in DESIGN.md §3).
  *
  * One context owns the state of one simulation on one CUDA device:

@@ -17,6 +17,11 @@
  * drho = rho - 1.  This is the same arithmetic (everything is linear in the rest state) and keeps
  * Pi^neq from being formed as a small difference of O(1/3) numbers.
  *
+ * A second forcing reading (A18, Guo-type time-centred forcing; tslb_ref.h TSLB_REF_FORCING_GUO) is
+ * implemented beside the kick of A9: collide_guo() / step_once() branches marked GUO.  The paper
+ * is silent on how the force enters; A18 is pinned by the published scheme's moment conditions,
+ * momentum balance, closed-form forced flows and a numpy restatement (tests/test_oracle_forcing.py).
+ *
  * Parity pins: tests/test_oracle_*.py.  Unpinned by the paper: the inflow/outflow details
  * (A10, A11) -- "parity unpinned" for those two planes; they are checked for boundedness,
  * inlet mass flux and oracle<->GPU agreement only.
