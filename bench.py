@@ -183,6 +183,16 @@ def oracle_sample(cfg_name, steps):
     return nodes * steps / dt / 1e9, ref.num_threads(), desc, dt / steps
 
 
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -195,7 +205,8 @@ def run_reference(args):
            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": sps * 1e3,
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
            "config": {"workload": desc, "grid": [nx, ny, nz]},
-           "cpu_baseline": {"value": glups, "unit": "GLUPS", "cores": threads, "kind": "oracle", "sample": sample},
+           "cpu_baseline": {"value": glups, "unit": "GLUPS", "cores": threads, "kind": "oracle", "sample": sample,
+                            "cpu_model": cpu_model()},
            "e2e": {"value": glups, "unit": "GLUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
            "gpu_launches": 0}
     print(json.dumps(out))
@@ -423,7 +434,8 @@ def main():
     cpu = None
     if not args.no_cpu:
         g, threads, sample, _ = oracle_sample(args.config, 6)
-        cpu = {"value": g, "unit": "GLUPS", "cores": threads, "kind": "oracle", "sample": sample}
+        cpu = {"value": g, "unit": "GLUPS", "cores": threads, "kind": "oracle", "sample": sample,
+               "cpu_model": cpu_model()}
 
     out = {"metric": "GLUPS (fused flow+phase-field step)", "value": glups, "unit": "GLUPS", "n_gpus": world,
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
