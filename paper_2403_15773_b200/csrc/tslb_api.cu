@@ -12,7 +12,6 @@
 #include "../../include/tslb.h"
 #include "tslb_generic.cuh"
 #include "tslb_tiled.cuh"
-#include "tslb_tiled_ws.cuh"
 
 #include <type_traits>
 
@@ -137,7 +136,6 @@ struct tslb_ctx {
   int stat_every = 0;          // 0: off
   long long stat_n = 0;        // samples accumulated
   TiledPlan tiled;             // TMA descriptors etc.
-  bool use_ws = false;         // warp-specialised variant of the tiled kernel (fp32, two-component)
   std::string err;
   std::string kname;
 
@@ -225,13 +223,7 @@ int step_typed(tslb_ctx *c, int nsteps) {
     StepParams<T> P = make_step_params<T>(c, c->cur, c->cur ^ 1);
     int rc;
     if (c->v.kernel == TSLB_KERNEL_TILED) {
-      cudaError_t e;
-      if constexpr (std::is_same<T, float>::value && TSLB_F32_TX == 32 && TSLB_TY == 8) {
-        e = c->use_ws ? launch_tiled_ws<32, 8>(c->tiled, P, c->cur, c->p.hermite_order, c->stream)
-                      : launch_tiled<T>(c->tiled, P, c->cur, c->p.hermite_order, c->p.two_component != 0, c->stream);
-      } else {
-        e = launch_tiled<T>(c->tiled, P, c->cur, c->p.hermite_order, c->p.two_component != 0, c->stream);
-      }
+      cudaError_t e = launch_tiled<T>(c->tiled, P, c->cur, c->p.hermite_order, c->p.two_component != 0, c->stream);
       c->launches += (c->v.jet_lo || c->v.out_hi) ? 2 : 1;   // + the boundary-plane kernel with inflow/outflow
       rc = (e == cudaSuccess) ? TSLB_OK : c->cuda_fail(e, "launch_tiled");
     } else {
@@ -439,12 +431,7 @@ int tslb_create(const tslb_params *p, tslb_ctx **out) {
       delete c;
       return TSLB_ECUDA;
     }
-    if (p->precision == TSLB_F32 && p->two_component && TSLB_F32_TX == 32 && TSLB_TY == 8 && p->nx % 32 == 0 &&
-        p->ny % 8 == 0 && !v.slab) {
-      const char *env = getenv("TSLB_WS");
-      c->use_ws = env ? atoi(env) != 0 : false;
-    }
-    c->kname = c->use_ws ? "tiled-ws" + c->tiled.name.substr(5) : c->tiled.name;
+    c->kname = c->tiled.name;
   } else {
     c->kname = p->forcing == TSLB_FORCING_GUO ? "generic-guo" : "generic";
   }

@@ -3,31 +3,37 @@
 // Work decomposition.  A CTA owns an x-y tile of TX x TY nodes and MARCHES along z
 // over a chunk of planes.  Per plane k it receives, by TMA (cp.async.bulk.tensor, one 4-D box for
 // the ten moment arrays and one 3-D box for phi, completion on an mbarrier), the old moments of
-// plane k on tile+halo and the old phi of plane k+1 into shared-memory rings, prefetched two planes
-// ahead.  Every thread owns TWO x-adjacent nodes (packed fp32 math, tslb_pair.cuh).
+// plane k on tile+halo and the old phi of plane k+1 into 3-stage shared-memory rings, prefetched
+// three planes ahead.  Every thread owns TWO x-adjacent nodes (packed fp32 math, tslb_pair.cuh).
 //
 // The 27-neighbour pull of PAPER.md:98 eq. 6 / Fig. 1 is evaluated in the tensor-product Hermite
 // basis (tslb_math.cuh) as three 1-D three-point passes:
-//   x-pass  (segment 1)  K_abc (17 per node, evaluated once) in push form: a+ / a- cross to the
-//                        neighbouring lane inside the warp -> X^p_bc (24 per node, registers);
-//   y-push  (seg. 1->2)  every row forms, per (p,c), the combination a+ it sends to the row above,
-//                        a- it sends to the row below and a0 it keeps: only 9+9 values per node
-//                        cross shared memory (not 24 x 3 rows) -> Y^pq_c (18, registers);
-//   z-push  (segment 2)  Y^pq_c of source plane k is pushed into the register accumulators of
-//                        the destination planes k-1, k, k+1 (two live accumulator sets);
+//   x-pass  K_abc (17 per node, evaluated once) in push form: a+ / a- cross to the neighbouring
+//           lane inside the warp -> X^p_bc (24 per node, registers);
+//   y-push  every row forms, per (p,c), the combination a+ it sends to the row above, a- it sends
+//           to the row below and a0 it keeps: 9+9 values per node cross shared memory, in a
+//           double-buffered field that the neighbouring rows read ONE ITERATION LATER -> Y^pq_c;
+//   z-push  Y^pq_c of source plane k-1 is pushed into the register accumulators of the destination
+//           planes k-2, k-1, k (two live accumulator sets);
 // so each stored moment is read from HBM once and the populations never exist in memory.
-// The phase-field half (eqs. 20-24) runs in the same kernel from the phi ring:
-// y-z pre-combinations T,U,V of phi (aux warps), G and n = G/(|G|+eps) on tile+1 into a 3-plane
-// ring, z-combinations of n, kappa = -div n, the kick, and the D3Q7 update assembled from
-// per-plane fluxes -- phi, grad(phi), n and kappa never touch HBM.
+// The phase-field half (eqs. 20-24) runs in the same kernel from the phi ring.
+// Every thread keeps, for its own node pair, the in-plane combinations D_x S_y phi, S_x D_y phi,
+// S_x S_y phi of the last three planes in registers, so G = grad(phi) and n = G/(|G|+eps) need nine
+// shared-memory loads per plane and no intermediate array; what crosses shared memory are the
+// z-combined normals (for kappa = -div n) and the D3Q7 fluxes phi +- q each node sends to its four
+// in-plane neighbours (push form) -- phi, grad(phi), n and kappa never touch HBM.
 //
-// Thread roles: TY "compute" rows own the tile; 4 "aux" rows: two do the x-pass of the two halo rows,
-// two the phi pre-combinations, all four the ring of the n field.  Two __syncthreads per plane.
+// Thread roles: TY/2 "compute" warps own the tile (two rows each); one warp does the x-pass and the
+// phase geometry of the two halo rows; 2 RY lanes of a last warp own the two halo columns (their
+// x-pass terms one plane ahead, their phase geometry) and its last lane issues the TMA loads.
+// Everything a thread reads from another warp was written one iteration earlier into the other half
+// of a double buffer: ONE __syncthreads per plane.
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <string>
+#include <type_traits>
 
 #include "../../include/tslb.h"
 #include "tslb_generic.cuh"
@@ -69,41 +75,61 @@ template <typename T, int TX_, int TY_, bool TWO>
 struct TileCfg {
   static constexpr int TX = TX_, TY = TY_;
   static constexpr int LX = TX / 2;        // threads per row (two nodes each)
+  static_assert(LX == 16 && TY % 4 == 0, "a warp owns two rows of 16 node pairs; a phase warp four rows");
   // left/right staged halo columns.  2 are needed; the TMA box row must be a multiple of 32 bytes
   // (16-byte-odd rows raised "illegal instruction" on B200), so fp32 stages 4.
   static constexpr int HL = sizeof(T) == 4 ? 4 : 2;
   static constexpr int RX = TX + 2 * HL;   // staged columns x0-HL .. x0+TX+HL-1
   static constexpr int RY = TY + 2;        // staged moment rows y0-1 .. y0+TY   ("region rows")
   static constexpr int RYP = TY + 4;       // staged phi rows y0-2 .. y0+TY+1
-  static constexpr int S = 3;              // moment ring (planes k-1, k, k+1)
-  static constexpr int SP = 4;             // phi ring
-  static constexpr int NR = 3;             // ring of n planes
-  // thread rows: TY compute rows + 4 aux rows (2 do the x-pass of the halo rows, 2 the phi
-  // pre-combinations; all 4 the ring of n).  TY + 4 warps divide evenly over the 4 schedulers.
-  static constexpr int NTHREADS = LX * (TY + 4);
-  static constexpr int NAUX = 4 * LX;
-  static constexpr int NYP = 9;            // y-push fields per direction: (p,c)
+  static constexpr int S = 3;              // TMA ring depth (group = moments of plane k + phi of plane k+2)
+  // warp roles: NWF flow warps (two tile rows each), the halo-row warp, the halo-column warp, and (two-
+  // component) NWP phase warps that own the phase field of four tile rows each
+  static constexpr int NWF = TY / 2;
+  static constexpr int NWP = TWO ? TY / 4 : 0;
+  static constexpr int W_HALO = NWF, W_COL = NWF + 1, W_PH0 = NWF + 2;
+  static constexpr int NTHREADS = 32 * (NWF + 2 + NWP);
+  static constexpr int NXPASS = 32 * (NWF + 1);          // threads that take part in the x-pass / y-push
+  static_assert(2 * RY < 32, "the halo-column warp has one lane per halo-column node and a spare lane");
+  static constexpr int NYP = 9;            // y-push fields per direction: (c,p)
+  static constexpr int ZW = TX + 4;        // columns x0-2 .. x0+TX+1 of a z-combined-normal array
+  static constexpr int FQW = LX + 2;       // node pairs per region row incl. the two halo-column pairs
   static constexpr size_t al(size_t b) { return (b + 127) / 128 * 128; }
   static constexpr size_t MOM_BYTES = (size_t)10 * RY * RX * sizeof(T);   // one TMA box
   static constexpr size_t PHI_BYTES = (size_t)RYP * RX * sizeof(T);
   static constexpr size_t MOM_STAGE = al(MOM_BYTES);
   static constexpr size_t PHI_STAGE = al(PHI_BYTES);
-  static constexpr size_t PLANE = al((size_t)RY * RX * sizeof(T));        // one region-plane array
-  static constexpr size_t YP_FIELD = al((size_t)RY * TX * sizeof(T));
+  // Exchange arrays, in ELEMENTS.  Everything that one warp writes and another reads one iteration later
+  // lives in a block that exists twice (index = plane parity), all arrays at the same offsets, so that one
+  // register (parity x block size) selects the half.
+  static constexpr int ZCE = RY * ZW;      // x-combined z-combinations of n: region rows x ZW columns
+  static constexpr int ZLE = 2 * RY + 4;   // the same z-combinations, raw, on the two halo columns
+  static constexpr int GQE = RY * TX;      // region rows x tile columns
+  static constexpr int FQE = RY * FQW;     // one scalar per node pair
+  static constexpr int TLE = TY * TX;      // tile nodes
+  static constexpr int XHE = 2 * 8 * RY;   // [2 sides][8 groups][RY]
+  static constexpr int B_ZC = 0;                                 // [3]  D_x S_z n_x, S_x S_z n_y, S_x d_z n_z
+  static constexpr int B_ZL = B_ZC + (TWO ? 3 * ZCE : 0);        // [3]  S_z n_x, S_z n_y, d_z n_z on the halo columns
+  static constexpr int B_ZZ = B_ZL + (TWO ? 3 * ZLE : 0);        // [3]  zeros (what the lanes off the tile edge read)
+  static constexpr int B_GQ = B_ZZ + (TWO ? 3 * ZLE : 0);        // [2]  phi + q_y, phi - q_y
+  static constexpr int B_FQ = B_GQ + (TWO ? 2 * GQE : 0);        // [2]  (phi + q_x).y, (phi - q_x).x per pair
+  static constexpr int B_KF = B_FQ + (TWO ? 2 * FQE : 0);        // [3]  F = sigma kappa grad(phi), phase -> flow
+  static constexpr int B_GR = B_KF + (TWO ? 3 * TLE : 0);        // [3]  grad(phi), private to the owning phase thread
+  static constexpr int B_PH = B_GR + (TWO ? 3 * TLE : 0);        // [1]  own phi, private to the owning phase thread
+  static constexpr int B_XH = B_PH + (TWO ? TLE : 0);            // x-pass terms of the two halo columns
+  static constexpr int BUF = (B_XH + XHE + 3) / 4 * 4;           // elements per half
+  static_assert(ZCE % 2 == 0 && ZLE % 2 == 0 && GQE % 2 == 0 && FQE % 2 == 0, "pair alignment");
+  static constexpr int YPF = TY * TX;      // y-push field: TY sending rows
   static constexpr size_t OFF_MOM = 0;
   static constexpr size_t OFF_PHI = OFF_MOM + S * MOM_STAGE;
-  static constexpr size_t OFF_TUV = OFF_PHI + (TWO ? SP * PHI_STAGE : 0);  // T, U, V of plane k
-  static constexpr size_t OFF_NRM = OFF_TUV + (TWO ? 3 * PLANE : 0);       // n ring [NR][3]
-  static constexpr size_t OFF_ZC = OFF_NRM + (TWO ? NR * 3 * PLANE : 0);   // S_z n_x, S_z n_y, d_z n_z
-  static constexpr size_t OFF_AP = OFF_ZC + (TWO ? 3 * PLANE : 0);         // y-push, upward  [9]
-  static constexpr size_t OFF_AM = OFF_AP + NYP * YP_FIELD;                // y-push, downward [9]
-  // x exchange.  Inside a warp the a+ of each pair's second node / a- of its first node cross
-  // through the warp's OWN first row of the y-push fields 0..7 (dead at that time).  Only the terms
-  // of the two halo columns x0-1 (a+) and x0+TX (a-) need storage of their own: [2][8][RY].
-  static constexpr size_t XH_BYTES = al((size_t)2 * 8 * RY * sizeof(T));
-  static constexpr size_t OFF_XH = OFF_AM + NYP * YP_FIELD;
-  static constexpr size_t OFF_BAR = OFF_XH + XH_BYTES;
+  static constexpr size_t OFF_BUF = OFF_PHI + (TWO ? S * PHI_STAGE : 0);    // [2][BUF]
+  // y-push fields: a+ of region rows 0..TY-1 and a- of region rows 2..TY+1 (written and read inside one
+  // iteration, between the x-pass barrier and the CTA barrier)
+  static constexpr size_t OFF_AP = OFF_BUF + (size_t)2 * BUF * sizeof(T);   // [9]
+  static constexpr size_t OFF_AM = OFF_AP + (size_t)NYP * YPF * sizeof(T);  // [9]
+  static constexpr size_t OFF_BAR = OFF_AM + (size_t)NYP * YPF * sizeof(T);
   static constexpr size_t SMEM_BYTES = OFF_BAR + 64;
+  static constexpr int CTAS_PER_SM = SMEM_BYTES <= 113 * 1024 ? 2 : 1;
 };
 
 struct TiledMaps {
@@ -120,6 +146,17 @@ __device__ __forceinline__ double rcp1(double s) { return 1.0 / s; }
 __device__ __forceinline__ float sqrt1(float s) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(s)); return r; }
 __device__ __forceinline__ double sqrt1(double s) { return sqrt(s); }
 template <typename T> __device__ __forceinline__ Pair<T> prcp(Pair<T> a) { return Pair<T>(rcp1(a.x), rcp1(a.y)); }
+
+// predicated shared-memory pair store (kept as ONE predicated instruction: a branch around a store
+// costs a convergence barrier per store in the x-pass)
+__device__ __forceinline__ void sts_pair_if(bool p, float *a, Pair<float> v) {
+  asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %0, 0;\n@q st.shared.v2.f32 [%1], {%2, %3};\n}"
+               ::"r"((int)p), "r"(smem_u32(a)), "f"(v.x), "f"(v.y) : "memory");
+}
+__device__ __forceinline__ void sts_pair_if(bool p, double *a, Pair<double> v) {
+  asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %0, 0;\n@q st.shared.v2.f64 [%1], {%2, %3};\n}"
+               ::"r"((int)p), "r"(smem_u32(a)), "d"(v.x), "d"(v.y) : "memory");
+}
 
 // The 1-D three-point operator of the tensor-product basis in PUSH form.  A source
 // node holding the un-normalised Hermite coefficients g_0, g_1, g_2 (index along this axis) sends
@@ -153,336 +190,380 @@ __device__ __forceinline__ void pull3s(T l, T upy, T dnx, T r, V a0, V &W0, V &W
   W2 = pfma(W0, T(2.0 / 3.0), pneg(a0));
 }
 
+// Per-node-pair state of the phase-field half that a thread carries from plane to plane in registers.
+// At the start of iteration k (the newest phi plane seen is k+1):
+template <typename T>
+struct PhaseState {
+  typedef Pair<T> V;
+  V P1b, P2b, P3b;   // D_x S_y phi, S_x D_y phi, S_x S_y phi of plane k+1
+  V A1, A2;          // w1 P(k) + w0 P(k+1) of the first two: G(k+1) = A + w1 P(k+2)
+  V D3;              // -1/2 P3(k):                             G_z(k+1) = D3 + 1/2 P3(k+2)
+  V nB[3];           // n(k)
+  V ZA, ZB, DZ;      // w1 n_x(k-1) + w0 n_x(k), the same of n_y, -1/2 n_z(k-1): z-combinations of plane k in the making
+  V acc, cup;        // phi'(k-1) in the making: phi/4 + (own cross terms + up(k-2))/8;  up(k-1)
+  __device__ __forceinline__ void clear() {
+    const V z(T(0));
+    P1b = P2b = P3b = A1 = A2 = D3 = ZA = ZB = DZ = acc = cup = z;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) nB[a] = z;
+  }
+};
+
+template <int N> using IC = std::integral_constant<int, N>;
+
+// Where a node pair sits in the staged arrays of the CTA: offset of its row r in a staged plane, staged
+// column c0 of its first node, the two outer columns (clamped: unused halves), its offsets in the
+// z-combined-normal, flux-scalar, tile-column and tile arrays.
+struct PairGeom {
+  int oP, c0, cl, cr, oZ, oF, oG, oT;
+};
+
+// Store the fields of MASK (bit m = field m) of one node pair of plane j: the node itself, its periodic
+// ghost images (edge tiles only) and, on a slab face, the same into the neighbour slab's ghost planes
+// through its peer pointers (phi from the two planes next to the face, the moments from the face
+// plane).  The field arrays of a buffer are equally spaced (fs elements).
+template <typename T, unsigned MASK, bool SLAB>
+__device__ __forceinline__ void store_pair(const StepParams<T> &P, const Pair<T> *o, int j, long long o00, int gx, int gy,
+                                           bool edge, long long fs) {
+  typedef Pair<T> V;
+  const Layout &L = P.L;
+  const long long zo = (long long)j * L.plane;
+  {
+    T *p = P.out.f[0] + zo + o00;
+    int last = 0;
+#pragma unroll
+    for (int m = 0; m < NF_MAX; ++m)
+      if (MASK >> m & 1u) { p += (m - last) * fs; last = m; *reinterpret_cast<V *>(p) = o[m]; }
+  }
+  const bool push = SLAB && ((j < 2 && P.nb[0].f[0]) || (j >= L.nz - 2 && P.nb[1].f[0]));
+  if (edge || push) {
+    const int gxg = gx < 2 ? gx + L.nx : (gx >= L.nx - 2 ? gx - L.nx : gx);
+    const int gyg = gy < GY ? gy + L.ny : (gy >= L.ny - GY ? gy - L.ny : gy);
+    const long long o10 = L.idx(gxg, gy, 0), o01 = L.idx(gx, gyg, 0), o11 = L.idx(gxg, gyg, 0);
+    if (gxg != gx || gyg != gy) {
+#pragma unroll 1
+      for (int im = 0; im < 3; ++im) {       // one copy of the store code: x image, y image, corner
+        if (im == 0 ? gxg == gx : (im == 1 ? gyg == gy : (gxg == gx || gyg == gy))) continue;
+        const long long og = zo + (im == 0 ? o10 : (im == 1 ? o01 : o11));
+#pragma unroll
+        for (int m = 0; m < NF_MAX; ++m)
+          if (MASK >> m & 1u) *reinterpret_cast<V *>(P.out.f[m] + og) = o[m];
+      }
+    }
+    if (push) {
+#pragma unroll 1
+      for (int side = 0; side < 2; ++side) {
+        const int depth = side == 0 ? j : L.nz - 1 - j;
+        if (!P.nb[side].f[0] || depth > 1) continue;
+        const long long zn = (long long)(j + P.nb_dz[side]) * L.plane;
+#pragma unroll 1
+        for (int im = 0; im < 4; ++im) {     // the node itself, then its x / y / corner images
+          if (im == 1 ? gxg == gx : (im == 2 ? gyg == gy : (im == 3 && (gxg == gx || gyg == gy)))) continue;
+          const long long og = zn + (im == 0 ? o00 : (im == 1 ? o10 : (im == 2 ? o01 : o11)));
+#pragma unroll
+          for (int m = 0; m < NF_MAX; ++m)
+            if ((MASK >> m & 1u) && (depth == 0 || m == F_PHI)) *reinterpret_cast<V *>(P.nb[side].f[m] + og) = o[m];
+        }
+      }
+    }
+  }
+}
+constexpr unsigned FM_U = 0xEu, FM_RHOPI = 0x3F1u, FM_FLOW = 0x3FFu, FM_PHI = 0x400u;   // field masks
+
 // ------------------------------------------------------------------ the kernel
-// SLAB: the context is a z-slab (halo faces, ghost planes, halo push).  A separate instantiation:
-// the single-GPU kernel's loop body sits at the 32 KB instruction-cache limit and must not grow.
+// SLAB: the context is a z-slab (halo faces, ghost planes, halo push).  A separate instantiation
+// keeps the single-GPU kernel's loop body small (instruction cache).
+//
+// Schedule.  Iteration k (k = z0-4 .. z1+1 for the chunk [z0, z1)) ends with the ONE CTA barrier:
+//   flow warps   A  K, x-pass and y-push terms of plane k (+ the halo-row warp for the two halo rows);
+//                   a barrier among these five warps only;
+//                C  y-pull of plane k, z-push: the flow moments of plane k-1 are complete; store rho' and
+//                   Pi^neq' of plane k-1; kick u'(k-2) = u_b(k-2) + F(k-2)/rho' with the F the phase warps
+//                   wrote in iteration k-1; store u' of plane k-2;
+//   halo-col warp   x-pass terms of the two halo columns of plane k+1 (one iteration ahead); B for the
+//                   halo-column pairs and the halo-row pairs; its spare lane issues the TMA group of plane
+//                   k+3 after the barrier;
+//   phase warps  D  kappa(k-1) from the x-combined z-combinations of n written in iteration k-1;
+//                   F(k-1) = sigma kappa grad(phi) -> flow warps;
+//                B  P(k+2) from the phi ring, G(k+1), n(k+1); z-combinations of n of plane k, combined
+//                   along x; fluxes phi +- q of plane k; phi'(k-1), stored at once.
+// Everything a warp reads from another role was written one iteration earlier into the other half of
+// the double-buffered exchange block.  The iterations before z0-1 only run B (they start the three-plane
+// history of the phase geometry).
 template <typename T, int TX, int TY, int ORDER, bool TWO, bool SLAB>
-__global__ void __launch_bounds__((TX / 2) * (TY + 4), (TileCfg<T, TX, TY, TWO>::SMEM_BYTES <= 113 * 1024 ? 2 : 1))
+__global__ void __launch_bounds__(TileCfg<T, TX, TY, TWO>::NTHREADS, TileCfg<T, TX, TY, TWO>::CTAS_PER_SM)
 tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant__ TiledMaps M) {
   using C = TileCfg<T, TX, TY, TWO>;
   using V = Pair<T>;
-  constexpr int LX = C::LX, HL = C::HL, RX = C::RX, RY = C::RY, S = C::S, SP = C::SP, NR = C::NR;
-  constexpr int PL = (int)(C::PLANE / sizeof(T));       // elements per region-plane array
-  constexpr int YPF = (int)(C::YP_FIELD / sizeof(T));   // elements per y-push field
+  constexpr int LX = C::LX, HL = C::HL, RX = C::RX, RY = C::RY, S = C::S, ZW = C::ZW, FQW = C::FQW;
+  constexpr int ZCE = C::ZCE, ZLE = C::ZLE, GQE = C::GQE, FQE = C::FQE, TLE = C::TLE, YPF = C::YPF, BUF = C::BUF;
   constexpr int MF = RY * RX;                           // elements per moment field in a stage
   extern __shared__ __align__(128) unsigned char smem[];
   uint64_t *bars = reinterpret_cast<uint64_t *>(smem + C::OFF_BAR);
   auto mom_at = [&](int slot) { return reinterpret_cast<T *>(smem + C::OFF_MOM + slot * C::MOM_STAGE); };
   auto phi_at = [&](int slot) { return reinterpret_cast<T *>(smem + C::OFF_PHI + slot * C::PHI_STAGE); };
-  auto nrm_at = [&](int slot) { return reinterpret_cast<T *>(smem + C::OFF_NRM + slot * 3 * C::PLANE); };
-  T *s_tuv = reinterpret_cast<T *>(smem + C::OFF_TUV);
-  T *s_zc = reinterpret_cast<T *>(smem + C::OFF_ZC);
-  T *s_ap = reinterpret_cast<T *>(smem + C::OFF_AP);
+  T *s_buf = reinterpret_cast<T *>(smem + C::OFF_BUF);     // [2][BUF]
+  T *s_ap = reinterpret_cast<T *>(smem + C::OFF_AP);       // [9][YPF]
   T *s_am = reinterpret_cast<T *>(smem + C::OFF_AM);
-  T *s_xhl = reinterpret_cast<T *>(smem + C::OFF_XH);      // a+ of column x0-1   [8][RY]
-  T *s_xhr = s_xhl + 8 * RY;                                // a- of column x0+TX  [8][RY]
 
   const Layout &L = P.L;
   const int t = threadIdx.x;
-  const int lx = t % LX;
-  const int tr = t / LX;
-  const bool aux = tr >= TY;
-  const bool xrow = tr < TY + 2;                          // does an x-pass row
-  const int r = aux ? (tr == TY ? 0 : RY - 1) : tr + 1;   // region row (y = y0 - 1 + r)
-  const int c0 = HL + 2 * lx;                             // staged column of the pair's first node
-  const int oM = r * RX + c0;                             // offset of the pair in a region plane
-  const int oY = r * TX + 2 * lx;                         // offset of the pair in a y-push field
-  // region-plane offset of the ring column next to the pair for the lanes at the tile edge; one
-  // common (valid) word for all other lanes
-  const int eoff = lx == 0 ? oM - 1 : (lx == LX - 1 ? oM + 2 : RX + HL);
-  const int ia = (tr - TY) * LX + lx;                     // aux thread index
-  // x-exchange word of this lane: word (t & 31) of the y-push row owned by lane 0 of the warp
-  const int trf = (t & ~31) / LX;
-  const int oX = (trf < TY ? trf + 1 : (trf == TY ? 0 : RY - 1)) * TX + (t & 31);
+  const int lane = t & 31, wid = t >> 5;
+  const bool flow = wid < C::NWF;                         // owns the flow of two tile rows
+  const bool halow = wid == C::W_HALO;
+  const bool colw = wid == C::W_COL;
+  const int lx = lane & (LX - 1), hi = lane >> 4;
+  // region row (y = y0 - 1 + r) of the thread's (first) node pair and staged column of its first node
+  const int r = flow ? 2 * wid + 1 + hi
+                     : (halow ? (hi ? 0 : RY - 1)
+                              : (colw ? (lane < RY ? lane : (lane < 2 * RY ? lane - RY : 0)) : 4 * (wid - C::W_PH0) + 1 + hi));
+  const int cside = lane >= RY;                           // halo-column warp: 0 left, 1 right
+  const int c0 = colw ? (cside ? HL + TX : HL - 2) : HL + 2 * lx;
+  const int oM = r * RX + c0;                             // offset of the pair in a staged region plane
+  const int oT = (r - 1) * TX + 2 * lx;                   // ... in an array over the tile
   // Tile origin.  When nx (ny) is not a multiple of the tile, the last tile of the row (column) is
   // shifted back to end at the domain edge; it recomputes the overlap but stores only its own nodes.
   const int xs = (blockIdx.x % M.ntx) * TX, ys = (blockIdx.x / M.ntx) * TY;
   const int x0 = min(xs, L.nx - TX), y0 = min(ys, L.ny - TY);
   const int z0 = blockIdx.y * M.zc;
   const int z1 = min(z0 + M.zc, L.nz);
-  const int kb = z0 - 1;                 // first source plane
-  const int NG = z1 - kb + 1;            // load groups / x-pass planes: kb .. z1
-  const int NI = NG + 1;                 // iterations
+  // first iteration's plane: two-component chunks start the three-plane history of the phase geometry
+  // at z0-4; single-component chunks need one iteration for the halo columns before the first x-pass
+  const int kst = TWO ? z0 - 4 : z0 - 2;
+  const int kfirst = TWO ? kst : z0 - 1; // first plane that has a TMA group
+  const int NI = z1 - kst + 2;           // iterations: k = kst .. z1+1
 
   // plane coordinate in the tensor map: wrapped / clamped / ghost plane of a slab (zsrc), shifted
   // by the ghost planes below z = 0
   auto zmap = [&](int z) { return zsrc(P, z) + L.gz; };
-  // group g (relative index): moments of plane kb+g -> slot g%S, phi of plane kb+g+1 -> slot (g+2)%SP
-  auto issue = [&](int g) {
-    uint64_t *bar = &bars[g % S];
-    uint32_t bytes = (uint32_t)C::MOM_BYTES + (TWO ? (uint32_t)C::PHI_BYTES : 0u);
-    if (TWO && g == 0) bytes += 2u * (uint32_t)C::PHI_BYTES;
-    mbar_expect_tx(bar, bytes);
-    tma_load_4d(mom_at(g % S), &M.mom, bar, x0 - HL + GX, y0 - 1 + GY, zmap(kb + g), 0);
-    if (TWO) {
-      tma_load_3d(phi_at((g + 2) % SP), &M.phi, bar, x0 - HL + GX, y0 - 2 + GY, zmap(kb + g + 1));
-      if (g == 0) {
-        tma_load_3d(phi_at(0), &M.phi, bar, x0 - HL + GX, y0 - 2 + GY, zmap(kb - 1));
-        tma_load_3d(phi_at(1), &M.phi, bar, x0 - HL + GX, y0 - 2 + GY, zmap(kb));
-      }
-    }
+  // group of plane k: moments of plane k (source planes z0-1 .. z1) and phi of plane k+2 (planes
+  // z0-2 .. z1+1)
+  auto has_group = [&](int k) { return k <= z1 && k >= kfirst; };
+  auto issue = [&](int k, int slot) {
+    uint64_t *bar = &bars[slot];
+    const bool mom = k >= z0 - 1, phi = TWO && k < z1;
+    mbar_expect_tx(bar, (mom ? (uint32_t)C::MOM_BYTES : 0u) + (phi ? (uint32_t)C::PHI_BYTES : 0u));
+    if (mom) tma_load_4d(mom_at(slot), &M.mom, bar, x0 - HL + GX, y0 - 1 + GY, zmap(k), 0);
+    if (phi) tma_load_3d(phi_at(slot), &M.phi, bar, x0 - HL + GX, y0 - 2 + GY, zmap(k + 2));
   };
 
-  if (t == 0) {
+  const bool issuer = t == 32 * C::W_COL + 31;           // spare lane of the halo-column warp
+  if (issuer) {
     for (int s = 0; s < S; ++s) mbar_init(&bars[s], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    for (int s = 0; s < S; ++s)
+      if (has_group(kfirst + s)) issue(kfirst + s, s);
   }
+  if (TWO)   // the zero arrays that the lanes off the tile edge read in D
+    for (int e = t; e < 2 * 3 * ZLE; e += C::NTHREADS) s_buf[(e / (3 * ZLE)) * BUF + C::B_ZZ + e % (3 * ZLE)] = T(0);
   __syncthreads();
 
   const V omc(P.omc);
   const T w1 = T(1.0 / 6.0), w0 = T(2.0 / 3.0);
-  V accA[10], accB[10];     // Hermite moments being accumulated for planes k and k+1
-  V fl[10];                 // finished flow part of the plane completed in the previous iteration:
-                            // drho', u_b (3), Pi^neq' (6)
-  V A0[9];                  // this row's own y-push term a0 per (c,p), carried across the barrier
-  V nA[3], nB[3];           // own n of planes k-2 and k-1
-  V gA(T(0)), gB(T(0));     // own |G| of planes k-2 and k-1
-  V c_inpl(T(0)), c_upa(T(0)), c_upb(T(0)), c_rinv(T(1));
-#pragma unroll
-  for (int m = 0; m < 10; ++m) { accA[m] = V(T(0)); accB[m] = V(T(0)); fl[m] = V(T(0)); }
-#pragma unroll
-  for (int m = 0; m < 3; ++m) { nA[m] = V(T(0)); nB[m] = V(T(0)); }
+  const long long fs = P.out.f[1] - P.out.f[0];          // field arrays are equally spaced
 
-  // global store offsets of the pair (plane 0); the periodic ghost images of edge nodes
-  const int gx_ = x0 + 2 * lx, gy_ = y0 + tr;
-  const int gxg = gx_ < 2 ? gx_ + L.nx : (gx_ >= L.nx - 2 ? gx_ - L.nx : gx_);
-  const int gyg = gy_ < GY ? gy_ + L.ny : (gy_ >= L.ny - GY ? gy_ - L.ny : gy_);
-  const bool own = gx_ >= xs && gy_ >= ys;
-  const long long o00 = L.idx(gx_, gy_, 0), o10 = L.idx(gxg, gy_, 0), o01 = L.idx(gx_, gyg, 0), o11 = L.idx(gxg, gyg, 0);
+  // global coordinates / store offset (plane 0) of the thread's (first) pair
+  const int gx_ = x0 + 2 * lx, gy_ = y0 + r - 1;
+  const long long o00 = L.idx(gx_, gy_, 0);
+  const bool edge_tile = x0 == 0 || x0 + TX == L.nx || y0 < GY || y0 + TY > L.ny - GY;
 
-  // x-pass terms of the two halo columns x0-1 (its a+) and x0+TX (its a-) of every region row of
-  // the plane held in moment slot `slot`; done by the A1 aux threads one segment ahead.
-  auto halo_cols = [&](int slot) {
-    const int e = ia - 2 * LX;
-    if (e >= 0 && e < 2 * RY) {
-      const int rr = e >> 1, side = e & 1;
-      const T *p = mom_at(slot) + rr * RX + (side ? HL + TX : HL - 1);
-      T m[10], K[NK];
-#pragma unroll
-      for (int f = 0; f < 10; ++f) m[f] = p[f * MF];
-      hermite_coeffs<ORDER, T>(m[0], m[1], m[2], m[3], m[4], m[5], m[6], m[7], m[8], m[9], P.omc, K);
-      T gp[8], gm[8], g0;
-      push3<3, T, T>(K[K000], K[K100], K[K200], gp[0], gm[0], g0);
-      push3<3, T, T>(K[K010], K[K110], K[K210], gp[1], gm[1], g0);
-      push3<2, T, T>(K[K020], K[K120], K[K120], gp[2], gm[2], g0);
-      push3<3, T, T>(K[K001], K[K101], K[K201], gp[3], gm[3], g0);
-      push3<2, T, T>(K[K011], K[K111], K[K111], gp[4], gm[4], g0);
-      push3<1, T, T>(K[K021], K[K021], K[K021], gp[5], gm[5], g0);
-      push3<2, T, T>(K[K002], K[K102], K[K102], gp[6], gm[6], g0);
-      push3<1, T, T>(K[K012], K[K012], K[K012], gp[7], gm[7], g0);
-#pragma unroll
-      for (int g = 0; g < 8; ++g) {
-        if (side == 0) s_xhl[g * RY + rr] = gp[g];
-        else s_xhr[g * RY + rr] = gm[g];
-      }
+  // B: phase geometry and fluxes of one node pair (eqs. 20-24, readings A6-A8), iteration k.
+  // ROLE 0: a tile pair (finishes and stores phi'); 1: a halo-row pair; 2: a halo-column pair.
+  // bo / bn: element offsets of the exchange-block halves of plane parity k&1 / (k-1)&1.
+  auto phase_B = [&](auto role, auto drc, PhaseState<T> &st, const PairGeom &g0, int k, int s, int bo, int bn) {
+    constexpr int ROLE = decltype(role)::value, DR = decltype(drc)::value;   // DR: rows below the thread's first pair
+    const PairGeom g = {g0.oP + DR * RX, g0.c0, g0.cl, g0.cr, g0.oZ + DR * ZW, g0.oF + DR * FQW, g0.oG + DR * TX, g0.oT + DR * TX};
+    // in-plane combinations of phi(k+2) on rows r-1, r, r+1 (phi box rows r .. r+2): first along y on the
+    // own columns (c) and on the two outer columns (n = (c0-1, c0+2)), then along x
+    const T *pp = phi_at(s) + g.oP;
+    const V ca = lds_pair(pp + g.c0), cb = lds_pair(pp + RX + g.c0), cc = lds_pair(pp + 2 * RX + g.c0);
+    const V na(pp[g.cl], pp[g.cr]), nb(pp[RX + g.cl], pp[RX + g.cr]), nc(pp[2 * RX + g.cl], pp[2 * RX + g.cr]);
+    const V syc = pfma(cb, w0, (ca + cc) * w1), dyc = cc - ca;          // S_y phi, 2 D_y phi
+    const V syn = pfma(nb, w0, (na + nc) * w1), dyn = nc - na;
+    const V sws(syc.y, syc.x), swd(dyc.y, dyc.x);
+    const V P1n = (sws - syn) * V(T(0.5), T(-0.5));                     // D_x S_y phi(k+2)
+    const V P3n = pfma(syc, w0, (syn + sws) * w1);                      // S_x S_y phi(k+2)
+    const V P2n = pfma(dyc, T(1.0 / 3.0), (dyn + swd) * T(1.0 / 12.0)); // S_x D_y phi(k+2)
+    // G(k+1) = (S_z P1, S_z P2, D_z P3), n(k+1) = G/(|G| + eps)
+    const V gx = pfma(P1n, w1, st.A1), gy = pfma(P2n, w1, st.A2), gz = pfma(P3n, T(0.5), st.D3);
+    st.A1 = pfma(P1n, w0, st.P1b * w1); st.P1b = P1n;
+    st.A2 = pfma(P2n, w0, st.P2b * w1); st.P2b = P2n;
+    st.D3 = st.P3b * T(-0.5); st.P3b = P3n;
+    const V s2 = pfma(gz, gz, pfma(gy, gy, gx * gx));
+    const V gC(sqrt1(s2.x), sqrt1(s2.y));                               // |G|
+    const V ginv(rcp1(gC.x + T(1e-12)), rcp1(gC.y + T(1e-12)));         // reading A7
+    const V nCx = gx * ginv, nCy = gy * ginv, nCz = gz * ginv;
+    // z-combinations of n of plane k: a = S_z n_x, b = S_z n_y, c = d_z n_z ...
+    const V za = pfma(nCx, w1, st.ZA), zb = pfma(nCy, w1, st.ZB), zc = pfma(nCz, T(0.5), st.DZ);
+    if (ROLE == 2) {
+      // ... of the halo column itself (x0-1: second node of its pair; x0+TX: first node), raw
+      T *zl = s_buf + bo + C::B_ZL + cside * RY + 2 + r;
+      zl[0] = cside ? za.x : za.y; zl[ZLE] = cside ? zb.x : zb.y; zl[2 * ZLE] = cside ? zc.x : zc.y;
+    } else {
+      // ... combined along x for kappa(k) = -(D_x S_y a + S_x D_y b + S_x S_y c): the outer columns come
+      // from the neighbour lanes; the lanes at the tile edge take 0 (D adds the halo column's share)
+      auto outer = [&](V v) {
+        const T l = __shfl_up_sync(0xffffffffu, v.y, 1, LX), q = __shfl_down_sync(0xffffffffu, v.x, 1, LX);
+        return V(lx == 0 ? T(0) : l, lx == LX - 1 ? T(0) : q);
+      };
+      const V oa = outer(za), ob = outer(zb), oc = outer(zc);
+      T *zw = s_buf + bo + C::B_ZC + g.oZ;
+      sts_pair(zw, (V(za.y, za.x) - oa) * V(T(0.5), T(-0.5)));          // D_x a
+      sts_pair(zw + ZCE, pfma(zb, w0, (ob + V(zb.y, zb.x)) * w1));      // S_x b
+      sts_pair(zw + 2 * ZCE, pfma(zc, w0, (oc + V(zc.y, zc.x)) * w1));  // S_x c
     }
+    // a7 in push form: the node sends phi + q_a along +e_a and phi - q_a along -e_a,
+    // q_a = phi (4 u_a + gamma (1 - phi) n_a), of plane k
+    const T *mo = mom_at(s) + g.oP + g.c0;
+    V ph;                                                               // own phi(k)
+    if (ROLE == 0) {
+      // tile pairs keep their own phi(k), phi(k+1) in a private two-slot ring (slot = plane parity)
+      T *pr = s_buf + bo + C::B_PH + g.oT;
+      ph = lds_pair(pr);
+      sts_pair(pr, cb);
+    } else {
+      ph = st.acc; st.acc = st.cup; st.cup = cb;                        // (their acc / cup carry phi(k), phi(k+1))
+    }
+    const V a4 = ph * T(4);
+    const V bq = ph * pfma(ph, V(T(0)) - V(P.gamma), V(P.gamma));
+    const V qx = pfma(bq, st.nB[0], a4 * lds_pair(mo + F_UX * MF));
+    const V qy = pfma(bq, st.nB[1], a4 * lds_pair(mo + F_UY * MF));
+    st.ZA = pfma(nCx, w0, st.nB[0] * w1); st.nB[0] = nCx;
+    st.ZB = pfma(nCy, w0, st.nB[1] * w1); st.nB[1] = nCy;
+    const V fp = ph + qx, fm = ph - qx;
+    T *fq = s_buf + bo + C::B_FQ + g.oF;
+    fq[0] = fp.y; fq[FQE] = fm.x;
+    if (ROLE != 2) {
+      T *gq = s_buf + bo + C::B_GQ + g.oG;
+      sts_pair(gq, ph + qy);
+      sts_pair(gq + GQE, ph - qy);
+    }
+    if (ROLE == 0) {
+      const V qz = pfma(bq, st.nB[2], a4 * lds_pair(mo + F_UZ * MF));
+      // grad(phi) of plane k+1 for the kick two iterations on: private two-slot ring (slot = plane parity)
+      T *gr_ = s_buf + bn + C::B_GR + g.oT;
+      sts_pair(gr_, gx); sts_pair(gr_ + TLE, gy); sts_pair(gr_ + 2 * TLE, gz);
+      // phi'(k-1) = phi/4 + (in-plane arrivals of plane k-1 + up(k-2) + down(k)) / 8, stored at once
+      const T *fr = s_buf + bn + C::B_FQ + g.oF;
+      const T *gr = s_buf + bn + C::B_GQ + g.oG;
+      const V xin(fr[-1], fr[FQE + 1]);
+      const V yin = lds_pair(gr - TX) + lds_pair(gr + GQE + TX);
+      V o[NF_MAX];
+      o[F_PHI] = pfma((xin + yin) + (ph - qz), T(0.125), st.acc);
+      const int j = k - 1;
+      if (j >= z0 && j < z1 && gx_ >= xs && gy_ + DR >= ys && !((P.jet_lo && j == 0) || (P.out_hi && j == L.nz - 1)))
+        store_pair<T, FM_PHI, SLAB>(P, o, j, o00 + (long long)DR * L.px, gx_, gy_ + DR, edge_tile, fs);
+      st.acc = pfma(V(fm.y, fp.x) + st.cup, T(0.125), ph * T(0.25));
+      st.cup = ph + qz;
+    }
+    st.DZ = st.nB[2] * T(-0.5); st.nB[2] = nCz;
   };
-  // Ring slots of iteration i: moments i%S, phi(k-1) i%SP, n(k) i%NR.  Iterations -2 and -1 are the
-  // pipeline prologue run through the same code (first two TMA groups, halo columns of the first
-  // plane): one copy of issue() and halo_cols() keeps the loop inside the instruction cache.
-  int ms = S - 2, ps = SP - 2, ns = NR - 2;
-  uint32_t mph = 1;                      // mbarrier phase parity of slot ms (flips when ms wraps to 0)
-  for (int i = -2; i < NI; ++i) {
-    const int k = kb + i;
-    const bool act = (unsigned)i < (unsigned)NG;       // plane k is a source plane of this chunk
-    if (act) mbar_wait(&bars[ms], mph);
-    const int ms1 = ms == 0 ? S - 1 : ms - 1;          // moments of plane k-1
-    const int ns1 = ns == 0 ? NR - 1 : ns - 1;         // n of plane k-1
-    const int ns2 = ns1 == 0 ? NR - 1 : ns1 - 1;       // n of plane k-2
-    const T *phm = phi_at(ps);                         // phi(k-1)
-    const T *phc = phi_at((ps + 1) % SP);              // phi(k)
-    const T *php = phi_at((ps + 2) % SP);              // phi(k+1)
 
-    // =========================== segment 1 ===========================
-    if (TWO && !xrow && act) {
-      // A1: T = S_y S_z phi, U = d_y S_z phi, V = S_y d_z phi of plane k on the region rows
-      // one thread per column pair, marching down the rows with a 3-row window of S_z phi, d_z phi
-      const int a1 = ia - 2 * LX;
-      if (a1 < RX / 2) {
-        const int cp = 2 * a1;
-        V sz0, sz1, sz2, dz0, dz1, dz2;
-        auto zrow = [&](int prow, V &sz, V &dz) {
-          const V a = lds_pair(phm + prow * RX + cp), b = lds_pair(phc + prow * RX + cp), c = lds_pair(php + prow * RX + cp);
-          sz = pfma(b, w0, (a + c) * w1);
-          dz = (c - a) * T(0.5);
-        };
-        zrow(0, sz0, dz0);
-        zrow(1, sz1, dz1);
-#pragma unroll
-        for (int rr = 0; rr < RY; ++rr) {
-          zrow(rr + 2, sz2, dz2);
-          sts_pair(s_tuv + rr * RX + cp, pfma(sz1, w0, (sz0 + sz2) * w1));
-          sts_pair(s_tuv + PL + rr * RX + cp, (sz2 - sz0) * T(0.5));
-          sts_pair(s_tuv + 2 * PL + rr * RX + cp, pfma(dz1, w0, (dz0 + dz2) * w1));
-          sz0 = sz1; sz1 = sz2; dz0 = dz1; dz1 = dz2;
-        }
-      }
-    }
-    if (!aux && i >= 1) {
-      V phin(T(0)), ukx(T(0)), uky(T(0)), ukz(T(0));
-      const int j = k - 2;                         // plane finalised in this iteration
-      const bool fin = (j >= z0);                  // (j < z1 always: k <= z1 + 1)
-      if (TWO) {
-        // fluxes of plane k-1 (operands resident: moments slot ms1, phi(k-1) = phm, n(k-1) slot ns1)
-        const T *ph = phm + (r + 1) * RX + c0;
-        const T *mo = mom_at(ms1) + oM;
-        const T *nr = nrm_at(ns1) + oM;
-        // q = phi (4 c.u + gamma (1-phi) c.n): the neighbour sends phi + q along +e, phi - q along -e
-        const V gamv(P.gamma);
-        auto qterm = [&](V p, V u, V n) { return p * pfma(pfma(p, V(T(0)) - gamv, gamv), n, u * T(4)); };
-        const V pc = lds_pair(ph);
-        // x direction: node x gets g+(c0-1) + g-(c0+1), node x+1 gets g+(c0) + g-(c0+2)
-        const V uxc = lds_pair(mo + F_UX * MF);
-        // (q on the own columns and on the two outer columns c0-1, c0+2; mixed only at the end)
-        const V pn(ph[-1], ph[2]);
-        const V qO = qterm(pc, uxc, nB[0]);
-        const V qX = qterm(pn, V(mo[F_UX * MF - 1], mo[F_UX * MF + 2]), V(nr[-1], nr[2]));
-        V inpl((pn.x + qX.x) + (pc.y - qO.y), (pc.x + qO.x) + (pn.y - qX.y));
-        // y direction: rows r-1 (south, c_i = +e_y) and r+1 (north)
-        const V phs = lds_pair(ph - RX), phn_ = lds_pair(ph + RX);
-        const V qS = qterm(phs, lds_pair(mo + F_UY * MF - RX), lds_pair(nr + PL - RX));
-        const V qN = qterm(phn_, lds_pair(mo + F_UY * MF + RX), lds_pair(nr + PL + RX));
-        inpl = inpl + ((phs + qS) + (phn_ - qN));
-        inpl = pfma(inpl, T(0.125), pc * T(0.25));
-        // z direction: this plane's contribution to the planes above (up) and below (down)
-        const V qZ = qterm(pc, lds_pair(mo + F_UZ * MF), nB[2]);
-        const V up = pc + qZ, down = pc - qZ;
-        if (fin) {
-          // a7: phi'(j) = inpl(j) + up(j-1)/8 + down(j+1)/8       (eqs. 23-24)
-          phin = pfma(c_upa + down, T(0.125), c_inpl);
-          // a5: kappa(j) = -div n from the z-combined normals a = S_z n_x, b = S_z n_y, c = d_z n_z
-          // Own columns from shared memory; the outer columns c0-1 / c0+2 come from the neighbour
-          // lanes by shuffle (3x the LSU rate, no bank conflicts).  The lanes at the tile edge read
-          // the ring column instead: one unconditional load per term through a per-lane pointer
-          // (all other lanes read one common word: a broadcast), no divergence.
-          const T *za = s_zc + oM, *zb = za + PL, *zc_ = za + 2 * PL;
-          V own(T(0)), eO(T(0));
-#pragma unroll
-          for (int dy = -1; dy <= 1; ++dy) {
-            const T w = dy == 0 ? w0 : w1;
-            own = pfma(lds_pair(za + dy * RX), w, own);       // S_y a
-            eO = pfma(lds_pair(zc_ + dy * RX), w, eO);         // S_y c
-          }
-          const V dO = lds_pair(zb + RX) - lds_pair(zb - RX);  // 2 d_y b
-          const T *ze = s_zc + eoff;                           // ring column (edge lanes) / dummy
-          const T ea = w1 * (ze[-RX] + ze[RX]) + w0 * ze[0];
-          const T ec = w1 * (ze[2 * PL - RX] + ze[2 * PL + RX]) + w0 * ze[2 * PL];
-          const T eb = ze[PL + RX] - ze[PL - RX];
-          auto left = [&](T v, T e) { const T q = __shfl_up_sync(0xffffffffu, v, 1, LX); return lx == 0 ? e : q; };
-          auto right = [&](T v, T e) { const T q = __shfl_down_sync(0xffffffffu, v, 1, LX); return lx == LX - 1 ? e : q; };
-          const T al = left(own.y, ea), ar = right(own.x, ea);
-          const T bl = left(dO.y, eb), br = right(dO.x, eb);
-          const T cl = left(eO.y, ec), cr = right(eO.x, ec);
-          V kap(T(0.5) * (own.y - al), T(0.5) * (ar - own.x));                     // d/dx S_y a
-          kap.x += T(0.5) * (w1 * bl + w0 * dO.x + w1 * dO.y);                       // S_x d/dy b
-          kap.y += T(0.5) * (w1 * dO.x + w0 * dO.y + w1 * br);
-          kap.x += w1 * cl + w0 * eO.x + w1 * eO.y;                                  // S_x S_y c
-          kap.y += w1 * eO.x + w0 * eO.y + w1 * cr;
-          // a6: F = sigma kappa G, kappa = -div n, G = n (|G| + eps); u' = u_b + F / rho'
-          const V sc = (kap * (gA + V(T(1e-12)))) * c_rinv * (-P.sigma);
-          ukx = nA[0] * sc; uky = nA[1] * sc; ukz = nA[2] * sc;
-        }
-        c_upa = c_upb; c_upb = up; c_inpl = inpl;
-      }
-      if (fin && own && !((P.jet_lo && j == 0) || (P.out_hi && j == L.nz - 1))) {
-        // a9: store plane j (and its periodic ghost images)
-        V o[NF_MAX];
-        o[0] = fl[0];
-        o[1] = fl[1] + ukx; o[2] = fl[2] + uky; o[3] = fl[3] + ukz;
-#pragma unroll
-        for (int m = 4; m < 10; ++m) o[m] = fl[m];
-        o[10] = phin;
-        const long long zo = (long long)j * L.plane;
-#pragma unroll
-        for (int m = 0; m < (TWO ? 11 : 10); ++m) *reinterpret_cast<V *>(P.out.f[m] + zo + o00) = o[m];
-        if (gxg != gx_ || gyg != gy_) {          // periodic ghost images (edge tiles only)
-#pragma unroll 1
-          for (int im = 0; im < 3; ++im) {       // one copy of the store code: x image, y image, corner
-            if (im == 0 ? gxg == gx_ : (im == 1 ? gyg == gy_ : (gxg == gx_ || gyg == gy_))) continue;
-            const long long og = zo + (im == 0 ? o10 : (im == 1 ? o01 : o11));
-#pragma unroll
-            for (int m = 0; m < (TWO ? 11 : 10); ++m) *reinterpret_cast<V *>(P.out.f[m] + og) = o[m];
-          }
-        }
-        // halo push (slab faces only, off the common path): the same stores into the neighbour
-        // slab's ghost planes through its peer pointers -- phi from the two planes next to the
-        // face, the moments from the face plane
-        if (SLAB && ((j < 2 && P.nb[0].f[0]) || (j >= L.nz - 2 && P.nb[1].f[0]))) {
-#pragma unroll 1
-          for (int side = 0; side < 2; ++side) {
-            const int depth = side == 0 ? j : L.nz - 1 - j;
-            if (!P.nb[side].f[0] || depth > 1) continue;
-            const long long zn = (long long)(j + P.nb_dz[side]) * L.plane;
-#pragma unroll 1
-            for (int im = 0; im < 4; ++im) {     // the node itself, then its x / y / corner images
-              if (im == 1 ? gxg == gx_ : (im == 2 ? gyg == gy_ : (im == 3 && (gxg == gx_ || gyg == gy_)))) continue;
-              const long long og = zn + (im == 0 ? o00 : (im == 1 ? o10 : (im == 2 ? o01 : o11)));
-#pragma unroll
-              for (int m = 0; m < (TWO ? 11 : 10); ++m)
-                if (depth == 0 || m == F_PHI) *reinterpret_cast<V *>(P.nb[side].f[m] + og) = o[m];
-            }
-          }
-        }
-      }
-    }
-    if (xrow && act) {
-      // A2: x-pass of region row r of plane k in push form, then the y-push terms.  Each node's K is
-      // evaluated once; a+ / a- cross to the x-neighbour thread through shared memory (same warp).
-      V Xg[8][3];   // [group][p]
-      {
-        V m[10], K[NK];
-        const T *p = mom_at(ms) + oM;
-#pragma unroll
-        for (int f = 0; f < 10; ++f) m[f] = lds_pair(p + f * MF);
-        hermite_coeffs<ORDER, V>(m[0], m[1], m[2], m[3], m[4], m[5], m[6], m[7], m[8], m[9], omc, K);
-        V gp[8], gm[8], g0[8];
-        push3<3, V, T>(K[K000], K[K100], K[K200], gp[0], gm[0], g0[0]);   // (b,c) = (0,0)
-        push3<3, V, T>(K[K010], K[K110], K[K210], gp[1], gm[1], g0[1]);   // (1,0)
-        push3<2, V, T>(K[K020], K[K120], K[K120], gp[2], gm[2], g0[2]);   // (2,0)
-        push3<3, V, T>(K[K001], K[K101], K[K201], gp[3], gm[3], g0[3]);   // (0,1)
-        push3<2, V, T>(K[K011], K[K111], K[K111], gp[4], gm[4], g0[4]);   // (1,1)
-        push3<1, V, T>(K[K021], K[K021], K[K021], gp[5], gm[5], g0[5]);   // (2,1)
-        push3<2, V, T>(K[K002], K[K102], K[K102], gp[6], gm[6], g0[6]);   // (0,2)
-        push3<1, V, T>(K[K012], K[K012], K[K012], gp[7], gm[7], g0[7]);   // (1,2)
-        // lane l of the warp parks gp.y / gm.x at word l of the warp's first y-push row
-        T *xp = s_ap + oX, *xm = s_am + oX;
-#pragma unroll
-        for (int g = 0; g < 8; ++g) { xp[g * YPF] = gp[g].y; xm[g * YPF] = gm[g].x; }
-        __syncwarp();
-        // left / right neighbour's word, or the halo column's term for the lanes at the tile edge
-        const T *pl = lx == 0 ? s_xhl + r : xp - 1, *pr = lx == LX - 1 ? s_xhr + r : xm + 1;
-        const int sl = lx == 0 ? RY : YPF, sr = lx == LX - 1 ? RY : YPF;
-#pragma unroll
-        for (int g = 0; g < 8; ++g) {
-          pull3s<V, T>(pl[g * sl], gp[g].x, gm[g].y, pr[g * sr], g0[g], Xg[g][0], Xg[g][1], Xg[g][2]);
-        }
-        __syncwarp();
-      }
-      // y-push per (c, p): groups of c = 0: b = 0,1,2 -> g 0,1,2; c = 1: g 3,4,5; c = 2: b = 0,1 -> g 6,7
-#pragma unroll
-      for (int c = 0; c < 3; ++c)
-#pragma unroll
-        for (int p = 0; p < 3; ++p) {
-          V ap, am;
-          if (c < 2) push3<3, V, T>(Xg[3 * c][p], Xg[3 * c + 1][p], Xg[3 * c + 2][p], ap, am, A0[3 * c + p]);
-          else push3<2, V, T>(Xg[6][p], Xg[7][p], Xg[7][p], ap, am, A0[6 + p]);
-          sts_pair(s_ap + (3 * c + p) * YPF + oY, ap);
-          sts_pair(s_am + (3 * c + p) * YPF + oY, am);
-        }
-    }
+  // D: kappa(k-1) = -(S_y ax + D_y bx + S_y cx) from the x-combined z-combinations of n written in iteration
+  // k-1, plus the share of the halo column for the lanes at the tile edge (every other lane reads zeros
+  // through the same per-lane pointer: no divergence); F(k-1) = sigma kappa grad(phi)(k-1) -> flow warps.
+  auto phase_D = [&](auto drc, const PairGeom &g0, int bn, int eoff, V emask, T esign) {
+    constexpr int DR = decltype(drc)::value;
+    const PairGeom g = {0, 0, 0, 0, g0.oZ + DR * ZW, 0, 0, g0.oT + DR * TX};
+    const T *zr = s_buf + bn + C::B_ZC + g.oZ;
+    V kap = pfma(lds_pair(zr), w0, (lds_pair(zr - ZW) + lds_pair(zr + ZW)) * w1);                       // S_y D_x a
+    kap = pfma(lds_pair(zr + ZCE + ZW) - lds_pair(zr + ZCE - ZW), T(0.5), kap);                         // D_y S_x b
+    kap = pfma(lds_pair(zr + 2 * ZCE), w0, pfma(lds_pair(zr + 2 * ZCE - ZW) + lds_pair(zr + 2 * ZCE + ZW), w1, kap));
+    const T *ze = s_buf + bn + eoff + DR;
+    const T ea = w0 * ze[0] + w1 * (ze[-1] + ze[1]);                     // S_y a on the halo column
+    const T eb = ze[ZLE + 1] - ze[ZLE - 1];                              // 2 D_y b
+    const T ec = w0 * ze[2 * ZLE] + w1 * (ze[2 * ZLE - 1] + ze[2 * ZLE + 1]);
+    const T corr = esign * ea + T(1.0 / 12.0) * eb + w1 * ec;            // -+ a/2 (D_x), w1 b and w1 c (S_x)
+    kap = pfma(V(corr), emask, kap);
+    const V sc = kap * (-P.sigma);                                       // F = sigma kappa G, kappa = -kap
+    const T *gr_ = s_buf + bn + C::B_GR + g.oT;
+    T *kf = s_buf + bn + C::B_KF + g.oT;
+    sts_pair(kf, lds_pair(gr_) * sc);
+    sts_pair(kf + TLE, lds_pair(gr_ + TLE) * sc);
+    sts_pair(kf + 2 * TLE, lds_pair(gr_ + 2 * TLE) * sc);
+  };
+
+  // ring slot of this iteration's group (group kfirst sits in slot 0) and its mbarrier phase parity
+  int s = TWO ? 0 : S - 1;
+  uint32_t mph = TWO ? 0u : 1u;
+  // end of an iteration: the ONE CTA barrier; the group three planes ahead goes into the slot just read
+  auto iter_end = [&](int k) {
     __syncthreads();
-    if (t == 0 && i + 2 < NG) issue(i + 2);
+    if (issuer && k >= kfirst && has_group(k + S)) issue(k + S, s);
+    s = s == S - 1 ? 0 : s + 1;
+    if (s == 0) mph ^= 1u;
+  };
 
-    // =========================== segment 2 ===========================
-    if (!xrow && (unsigned)(i + 1) < (unsigned)NG) {
-      const int sl = ms == S - 1 ? 0 : ms + 1;
-      mbar_wait(&bars[sl], sl == 0 ? mph ^ 1u : mph);
-      halo_cols(sl);
-    }
-    if (act) {
-      if (!aux) {
-        // B2: finish the y-pass (a+ from the row below, a- from the row above, own a0) and z-push.
+  if (flow || halow) {
+    // ============================ flow warps and the halo-row warp ============================
+    V accA[10], accB[10];     // Hermite moments being accumulated for planes k and k+1
+    V ubx(T(0)), uby(T(0)), ubz(T(0)), rinv(T(1));   // u_b and 1/rho' of the plane completed last
+#pragma unroll
+    for (int m = 0; m < 10; ++m) { accA[m] = V(T(0)); accB[m] = V(T(0)); }
+    // y-push fields: a+ is stored at row index r (rows 0..TY-1 send one), a- at r-2 (rows 2..TY+1);
+    // a tile row r reads both at index r-1 (= oT)
+    const bool st_ap = r <= TY - 1, st_am = r >= 2;
+    const int oAP = r * TX + 2 * lx, oAM = oAP - 2 * TX;
+    // x-exchange word of this lane: word `lane` of a row of the y-push fields 0..7 that this warp is
+    // about to overwrite (a+ field: the warp's first sending row; a- field: its last)
+    T *const xp = s_ap + (flow ? 2 * wid + 1 : 0) * TX + lane, *const xm = s_am + (flow ? 2 * wid : TY - 1) * TX + lane;
+    for (int i = 0; i < NI; ++i) {
+      const int k = kst + i;
+      const int bo = (k & 1) * BUF;          // exchange-block half of this plane's parity
+      if (has_group(k)) mbar_wait(&bars[s], mph);
+      const bool src = k >= z0 - 1 && k <= z1;     // plane k is a source plane of this chunk
+      V A0[9];                               // own y-push term a0 per (c,p)
+      if (src) {
+        // A: x-pass of region row r of plane k in push form, then the y-push terms.  Each node's K is
+        // evaluated once; a+ / a- cross to the x-neighbour thread through shared memory (same warp).
+        const T *xh = s_buf + bo + C::B_XH;
+        V Xg[8][3];   // [group][p]
+        {
+          V m[10], K[NK];
+          const T *p = mom_at(s) + oM;
+#pragma unroll
+          for (int f = 0; f < 10; ++f) m[f] = lds_pair(p + f * MF);
+          hermite_coeffs<ORDER, V>(m[0], m[1], m[2], m[3], m[4], m[5], m[6], m[7], m[8], m[9], omc, K);
+          V gp[8], gm[8], g0[8];
+          push3<3, V, T>(K[K000], K[K100], K[K200], gp[0], gm[0], g0[0]);   // (b,c) = (0,0)
+          push3<3, V, T>(K[K010], K[K110], K[K210], gp[1], gm[1], g0[1]);   // (1,0)
+          push3<2, V, T>(K[K020], K[K120], K[K120], gp[2], gm[2], g0[2]);   // (2,0)
+          push3<3, V, T>(K[K001], K[K101], K[K201], gp[3], gm[3], g0[3]);   // (0,1)
+          push3<2, V, T>(K[K011], K[K111], K[K111], gp[4], gm[4], g0[4]);   // (1,1)
+          push3<1, V, T>(K[K021], K[K021], K[K021], gp[5], gm[5], g0[5]);   // (2,1)
+          push3<2, V, T>(K[K002], K[K102], K[K102], gp[6], gm[6], g0[6]);   // (0,2)
+          push3<1, V, T>(K[K012], K[K012], K[K012], gp[7], gm[7], g0[7]);   // (1,2)
+          // lane l of the warp parks gp.y / gm.x at word l of one of the warp's own y-push rows
+#pragma unroll
+          for (int g = 0; g < 8; ++g) { xp[g * YPF] = gp[g].y; xm[g * YPF] = gm[g].x; }
+          __syncwarp();
+          // left / right neighbour's word, or the halo column's term for the lanes at the tile edge
+          const T *pl = lx == 0 ? xh + r : xp - 1, *pr = lx == LX - 1 ? xh + 8 * RY + r : xm + 1;
+          const int sl = lx == 0 ? RY : YPF, sr = lx == LX - 1 ? RY : YPF;
+#pragma unroll
+          for (int g = 0; g < 8; ++g) {
+            pull3s<V, T>(pl[g * sl], gp[g].x, gm[g].y, pr[g * sr], g0[g], Xg[g][0], Xg[g][1], Xg[g][2]);
+          }
+          __syncwarp();
+        }
+        // y-push per (c, p): groups of c = 0: b = 0,1,2 -> g 0,1,2; c = 1: g 3,4,5; c = 2: b = 0,1 -> g 6,7
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+#pragma unroll
+          for (int p = 0; p < 3; ++p) {
+            V ap, am;
+            if (c < 2) push3<3, V, T>(Xg[3 * c][p], Xg[3 * c + 1][p], Xg[3 * c + 2][p], ap, am, A0[3 * c + p]);
+            else push3<2, V, T>(Xg[6][p], Xg[7][p], Xg[7][p], ap, am, A0[6 + p]);
+            sts_pair_if(st_ap, s_ap + (3 * c + p) * YPF + oAP, ap);
+            sts_pair_if(st_am, s_am + (3 * c + p) * YPF + oAM, am);
+          }
+      }
+      // the y-push terms of plane k are complete (flow warps and the halo-row warp only)
+      asm volatile("bar.sync 1, %0;" ::"n"(C::NXPASS) : "memory");
+      if (flow && src) {
+        // C: finish the y-pass of plane k (a+ from the row below, a- from the row above, own a0) and z-push
+        const T *yu = s_ap + oT, *yd = s_am + oT;
         V outm[10];
         // moment index of (p,q,rr)
         constexpr int MI[3][3][3] = {{{0, 3, 6}, {2, 9, -1}, {5, -1, -1}}, {{1, 8, -1}, {7, -1, -1}, {-1, -1, -1}}, {{4, -1, -1}, {-1, -1, -1}, {-1, -1, -1}}};
@@ -491,8 +572,8 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
           V Yq[3][3];   // [q][c]
 #pragma unroll
           for (int c = 0; c < 3; ++c) {
-            const V up = lds_pair(s_ap + (3 * c + p) * YPF + oY - TX);
-            const V dn = lds_pair(s_am + (3 * c + p) * YPF + oY + TX);
+            const V up = lds_pair(yu + (3 * c + p) * YPF);
+            const V dn = lds_pair(yd + (3 * c + p) * YPF);
             pull3<V, T>(up, dn, A0[3 * c + p], Yq[0][c], Yq[1][c], Yq[2][c]);
           }
 #pragma unroll
@@ -515,71 +596,118 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
             }
           }
         }
-        // a4: plane k-1 is complete: u_b = m'/rho', Pi^neq' = Pi' - rho' u_b u_b (Hermite form)
-        const V inv = prcp<T>(outm[0] + V(T(1)));
-        c_rinv = inv;
-        fl[0] = outm[0];
-        fl[1] = outm[1] * inv; fl[2] = outm[2] * inv; fl[3] = outm[3] * inv;
-        fl[4] = outm[4] - outm[1] * fl[1];
-        fl[5] = outm[5] - outm[2] * fl[2];
-        fl[6] = outm[6] - outm[3] * fl[3];
-        fl[7] = outm[7] - outm[1] * fl[2];
-        fl[8] = outm[8] - outm[1] * fl[3];
-        fl[9] = outm[9] - outm[2] * fl[3];
-      }
-      if (TWO) {
-        // B1: G = (d_x T, S_x U, S_x V), n = G/(|G|+eps) of plane k on tile+1 -> ring slot ns
-        T *nk = nrm_at(ns);
-        auto gn_pair = [&](int o, int ol, int orr, V nn[3], V &mag) {
-          const V tc = lds_pair(s_tuv + o), uc = lds_pair(s_tuv + PL + o), vc = lds_pair(s_tuv + 2 * PL + o);
-          const T tl = s_tuv[ol], tr_ = s_tuv[orr], ul = s_tuv[PL + ol], ur = s_tuv[PL + orr];
-          const T vl = s_tuv[2 * PL + ol], vr = s_tuv[2 * PL + orr];
-          const V gx(T(0.5) * (tc.y - tl), T(0.5) * (tr_ - tc.x));
-          const V gy(w1 * (ul + uc.y) + w0 * uc.x, w1 * (uc.x + ur) + w0 * uc.y);
-          const V gz(w1 * (vl + vc.y) + w0 * vc.x, w1 * (vc.x + vr) + w0 * vc.y);
-          const V s2 = pfma(gz, gz, pfma(gy, gy, gx * gx));
-          mag = V(sqrt1(s2.x), sqrt1(s2.y));                                  // |G|
-          const V inv(rcp1(mag.x + T(1e-12)), rcp1(mag.y + T(1e-12)));             // reading A7
-          nn[0] = gx * inv; nn[1] = gy * inv; nn[2] = gz * inv;
-          sts_pair(nk + o, nn[0]); sts_pair(nk + PL + o, nn[1]); sts_pair(nk + 2 * PL + o, nn[2]);
-        };
-        if (!aux) {
-          V nC[3], gC;
-          gn_pair(oM, oM - 1, oM + 2, nC, gC);
-          // z-combinations of the own normals for kappa(k-1)
-          sts_pair(s_zc + oM, pfma(nB[0], w0, (nA[0] + nC[0]) * w1));
-          sts_pair(s_zc + PL + oM, pfma(nB[1], w0, (nA[1] + nC[1]) * w1));
-          sts_pair(s_zc + 2 * PL + oM, (nC[2] - nA[2]) * T(0.5));
-#pragma unroll
-          for (int a = 0; a < 3; ++a) { nA[a] = nB[a]; nB[a] = nC[a]; }
-          gA = gB; gB = gC;
-        } else {
-          constexpr int PPR = TX / 2 + 2;                // pairs per full ring row: cols HL-2 .. HL+TX+1
-          constexpr int NT = 2 * PPR + 2 * TY;           // ring tasks
-          const T *n1 = nrm_at(ns1), *n2 = nrm_at(ns2);
-          for (int e = ia; e < NT; e += C::NAUX) {
-            int rr, c;
-            if (e < 2 * PPR) { rr = (e < PPR) ? 0 : RY - 1; c = HL - 2 + 2 * (e % PPR); }
-            else { const int q = e - 2 * PPR; rr = 1 + (q >> 1); c = (q & 1) ? HL + TX : HL - 2; }
-            const int o = rr * RX + c;
-            const int ol = c > 0 ? o - 1 : o, orr = c + 2 < RX ? o + 2 : o + 1;   // clamped; edge results unused
-            V nC[3], gC;
-            gn_pair(o, ol, orr, nC, gC);
-            const V a2 = lds_pair(n2 + o), a1 = lds_pair(n1 + o);
-            const V b2 = lds_pair(n2 + PL + o), b1 = lds_pair(n1 + PL + o);
-            const V c2 = lds_pair(n2 + 2 * PL + o);
-            sts_pair(s_zc + o, pfma(a1, w0, (a2 + nC[0]) * w1));
-            sts_pair(s_zc + PL + o, pfma(b1, w0, (b2 + nC[1]) * w1));
-            sts_pair(s_zc + 2 * PL + o, (nC[2] - c2) * T(0.5));
+        const bool mine = gx_ >= xs && gy_ >= ys;
+        V o[NF_MAX];
+        if (TWO) {
+          // a6: u'(k-2) = u_b + F / rho' with the F(k-2) of the phase warps; a9: store it
+          const int j = k - 2;
+          if (j >= z0 && mine && !((P.jet_lo && j == 0) || (P.out_hi && j == L.nz - 1))) {
+            const T *kf = s_buf + bo + C::B_KF + oT;
+            o[1] = pfma(lds_pair(kf), rinv, ubx);
+            o[2] = pfma(lds_pair(kf + TLE), rinv, uby);
+            o[3] = pfma(lds_pair(kf + 2 * TLE), rinv, ubz);
+            store_pair<T, FM_U, SLAB>(P, o, j, o00, gx_, gy_, edge_tile, fs);
           }
         }
+        // a4: plane k-1 is complete: u_b = m'/rho', Pi^neq' = Pi' - rho' u_b u_b (Hermite form)
+        rinv = prcp<T>(outm[0] + V(T(1)));
+        ubx = outm[1] * rinv; uby = outm[2] * rinv; ubz = outm[3] * rinv;
+        const int j = k - 1;
+        if (j >= z0 && mine && !((P.jet_lo && j == 0) || (P.out_hi && j == L.nz - 1))) {
+          o[0] = outm[0];
+          o[4] = outm[4] - outm[1] * ubx;
+          o[5] = outm[5] - outm[2] * uby;
+          o[6] = outm[6] - outm[3] * ubz;
+          o[7] = outm[7] - outm[1] * uby;
+          o[8] = outm[8] - outm[1] * ubz;
+          o[9] = outm[9] - outm[2] * ubz;
+          if (TWO) {
+            store_pair<T, FM_RHOPI, SLAB>(P, o, j, o00, gx_, gy_, edge_tile, fs);
+          } else {
+            o[1] = ubx; o[2] = uby; o[3] = ubz;
+            store_pair<T, FM_FLOW, SLAB>(P, o, j, o00, gx_, gy_, edge_tile, fs);
+          }
+        }
+      } else if (TWO && flow && k == z1 + 1) {
+        // the kick and the velocity of the chunk's last plane
+        const int j = k - 2;
+        if (gx_ >= xs && gy_ >= ys && !((P.jet_lo && j == 0) || (P.out_hi && j == L.nz - 1))) {
+          V o[NF_MAX];
+          const T *kf = s_buf + bo + C::B_KF + oT;
+          o[1] = pfma(lds_pair(kf), rinv, ubx);
+          o[2] = pfma(lds_pair(kf + TLE), rinv, uby);
+          o[3] = pfma(lds_pair(kf + 2 * TLE), rinv, ubz);
+          store_pair<T, FM_U, SLAB>(P, o, j, o00, gx_, gy_, edge_tile, fs);
+        }
       }
+      iter_end(k);
     }
-    __syncthreads();
-    ms = ms == S - 1 ? 0 : ms + 1;
-    if (ms == 0) mph ^= 1u;
-    ps = ps == SP - 1 ? 0 : ps + 1;
-    ns = ns == NR - 1 ? 0 : ns + 1;
+  } else if (colw) {
+    // ============================ halo-column warp ============================
+    // node pairs: lanes 0 .. 2 RY - 1 own the two halo columns; every lane owns a pair of the halo rows
+    PhaseState<T> pc, ph_;
+    pc.clear(); ph_.clear();
+    const int cl = c0 > 0 ? c0 - 1 : 0, cr = c0 + 2 < RX ? c0 + 2 : RX - 1;   // clamped: unused halves
+    const int rh = hi ? 0 : RY - 1, ch = HL + 2 * lx;
+    const PairGeom gc = {r * RX, c0, cl, cr, 0, r * FQW + (c0 - (HL - 2)) / 2, 0, 0};
+    const PairGeom gh = {rh * RX, ch, ch - 1, ch + 2, rh * ZW + 2 + 2 * lx, rh * FQW + 1 + lx, rh * TX + 2 * lx, 0};
+    for (int i = 0; i < NI; ++i) {
+      const int k = kst + i;
+      const int bo = (k & 1) * BUF, bn = BUF - bo;
+      if (has_group(k)) mbar_wait(&bars[s], mph);
+      if (k + 1 >= z0 - 1 && k + 1 <= z1) {
+        // x-pass terms of the two halo columns x0-1 (its a+) and x0+TX (its a-) of every region row of
+        // plane k+1 (moments in the next ring slot), one iteration ahead of the rows that use them
+        const int s1 = s == S - 1 ? 0 : s + 1;
+        mbar_wait(&bars[s1], s1 == 0 ? mph ^ 1u : mph);
+        if (lane < 2 * RY) {
+          const T *p = mom_at(s1) + r * RX + (cside ? HL + TX : HL - 1);
+          T m[10], K[NK];
+#pragma unroll
+          for (int f = 0; f < 10; ++f) m[f] = p[f * MF];
+          hermite_coeffs<ORDER, T>(m[0], m[1], m[2], m[3], m[4], m[5], m[6], m[7], m[8], m[9], P.omc, K);
+          T gp[8], gm[8], g0;
+          push3<3, T, T>(K[K000], K[K100], K[K200], gp[0], gm[0], g0);
+          push3<3, T, T>(K[K010], K[K110], K[K210], gp[1], gm[1], g0);
+          push3<2, T, T>(K[K020], K[K120], K[K120], gp[2], gm[2], g0);
+          push3<3, T, T>(K[K001], K[K101], K[K201], gp[3], gm[3], g0);
+          push3<2, T, T>(K[K011], K[K111], K[K111], gp[4], gm[4], g0);
+          push3<1, T, T>(K[K021], K[K021], K[K021], gp[5], gm[5], g0);
+          push3<2, T, T>(K[K002], K[K102], K[K102], gp[6], gm[6], g0);
+          push3<1, T, T>(K[K012], K[K012], K[K012], gp[7], gm[7], g0);
+          T *xh = s_buf + bn + C::B_XH + cside * 8 * RY + r;
+#pragma unroll
+          for (int g = 0; g < 8; ++g) xh[g * RY] = cside ? gm[g] : gp[g];
+        }
+      }
+      if (TWO && k <= z1) {
+        if (lane < 2 * RY) phase_B(IC<2>(), IC<0>(), pc, gc, k, s, bo, bn);
+        phase_B(IC<1>(), IC<0>(), ph_, gh, k, s, bo, bn);
+      }
+      iter_end(k);
+    }
+  } else {
+    // ============================ phase warps ============================
+    PhaseState<T> p0, p1;     // two node pairs: rows r and r + 2
+    p0.clear(); p1.clear();
+    const int oZ = r * ZW + 2 + 2 * lx, oF = r * FQW + 1 + lx, oG = r * TX + 2 * lx;
+    const PairGeom g0 = {r * RX, c0, c0 - 1, c0 + 2, oZ, oF, oG, oT};
+    // the halo column's z-combinations of n for the lanes at the tile edge (row r of the raw array of that
+    // side), zeros for every other lane; the lane's weights of that share
+    const int eoff = (lx == 0 ? C::B_ZL : (lx == LX - 1 ? C::B_ZL + RY : C::B_ZZ)) + 2 + r;
+    const V emask(lx == 0 ? T(1) : T(0), lx == LX - 1 ? T(1) : T(0));
+    const T esign = lx == 0 ? T(-0.5) : T(0.5);
+    for (int i = 0; i < NI; ++i) {
+      const int k = kst + i;
+      const int bo = (k & 1) * BUF, bn = BUF - bo;
+      if (has_group(k)) mbar_wait(&bars[s], mph);
+      if (k <= z1) {
+        if (k - 1 >= z0) { phase_D(IC<0>(), g0, bn, eoff, emask, esign); phase_D(IC<2>(), g0, bn, eoff, emask, esign); }
+        phase_B(IC<0>(), IC<0>(), p0, g0, k, s, bo, bn);
+        phase_B(IC<0>(), IC<2>(), p1, g0, k, s, bo, bn);
+      }
+      iter_end(k);
+    }
   }
 }
 
@@ -588,9 +716,12 @@ typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32
                                     const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
                                     CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
+constexpr int TSLB_MAX_DEVICES = 64;
+
 struct TiledPlan {
   std::string name;
   int precision = 0, tx = 0, ty = 0, zc = 0;
+  int device = 0;        // the context's device (kernel attributes are set once per device)
   TiledMaps maps[2];     // per source buffer
   bool two = false;
 };
@@ -620,7 +751,7 @@ inline bool tiled_supported(int precision, int nx, int ny, int nz) {
 
 inline bool tiled_plan_create(TiledPlan &pl, int precision, const Layout &L, void *fields[2][NF_MAX], int nfields,
                               int device, std::string &why) {
-  (void)device;
+  pl.device = device;
   PFN_encodeTiled enc = nullptr;
   cudaDriverEntryPointQueryResult qres;
   cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", (void **)&enc, cudaEnableDefault, &qres);
@@ -655,18 +786,18 @@ inline bool tiled_plan_create(TiledPlan &pl, int precision, const Layout &L, voi
     pl.maps[b].ntx = (L.nx + pl.tx - 1) / pl.tx;
     pl.maps[b].nty = (L.ny + pl.ty - 1) / pl.ty;
   }
-  // z chunking: every chunk pays a 3-plane pipeline prologue, and the grid runs in waves of
-  // (CTAs per SM) x (SM count): pick the chunk length that minimises waves x (zc + 3).
+  // z chunking: every chunk pays a 6-iteration pipeline prologue (three of them light), and the grid
+  // runs in waves of (CTAs per SM) x (SM count): pick the chunk length that minimises waves x (zc + 5).
   const long long tiles = (long long)pl.maps[0].ntx * pl.maps[0].nty;
   int nsm = 148;
   cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, device);
   const long long slots = (long long)nsm * (precision == TSLB_F32 ? 2 : 1);
   int zc = L.nz;
   long long best = -1;
-  for (int cand = 8; cand <= 128; cand *= 2) {
+  for (int cand = 8; cand <= 256; cand *= 2) {
     const int c = cand < L.nz ? cand : L.nz;
     const long long ctas = tiles * ((L.nz + c - 1) / c);
-    const long long cost = ((ctas + slots - 1) / slots) * (c + 3);
+    const long long cost = ((ctas + slots - 1) / slots) * (c + 5);
     if (best < 0 || cost < best) { best = cost; zc = c; }
   }
   if (const char *env = getenv("TSLB_ZCHUNK")) { int v = atoi(env); if (v > 0) zc = v; }
@@ -706,11 +837,11 @@ cudaError_t launch_tiled_t(TiledPlan &pl, const StepParams<T> &P, int src, int o
   do {                                                                                                \
     using Cf = TileCfg<T, TX, TY, TWOC>;                                                              \
     auto kern = tiled_step_kernel<T, TX, TY, ORD, TWOC, SL>;                                          \
-    static bool attr_set = false;                                                                     \
-    if (!attr_set) {                                                                                  \
+    static bool attr_set[TSLB_MAX_DEVICES] = {};   /* the attribute is per DEVICE */                  \
+    if (pl.device < 0 || pl.device >= TSLB_MAX_DEVICES || !attr_set[pl.device]) {                     \
       e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cf::SMEM_BYTES); \
       if (e != cudaSuccess) return e;                                                                 \
-      attr_set = true;                                                                                \
+      if (pl.device >= 0 && pl.device < TSLB_MAX_DEVICES) attr_set[pl.device] = true;                 \
     }                                                                                                 \
     kern<<<grid, Cf::NTHREADS, Cf::SMEM_BYTES, st>>>(P, M);                                           \
   } while (0)

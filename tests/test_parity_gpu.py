@@ -381,27 +381,3 @@ def test_device_pointers_and_torch_stream():
     for k in ("rho", "ux", "phi"):
         assert np.array_equal(md[k].cpu().numpy(), mh[k])
     assert np.array_equal(md["pineq"].cpu().numpy(), mh["pineq"])
-
-
-def test_warp_specialised_variant(monkeypatch):
-    """tiled_ws_kernel (TSLB_WS=1: flow / phase / aux warps, setmaxnreg) computes the same step."""
-    monkeypatch.setenv("TSLB_WS", "1")
-    prm = dict(nx=192, ny=24, nz=33, omega=1.9, two_component=True, sigma=0.01, interface_width=3.0)
-    d, r = oracle_run("tm%s" % ((192, 24, 33),), lambda: inputs.smooth_random(192, 24, 33, seed=5), prm, 10, tslb.F32)
-    g = tslb.Tslb(192, 24, 33, 1.9, precision=tslb.F32, kernel=tslb.KERNEL_TILED, **gpu_kwargs(prm))
-    assert g.kernel_name.startswith("tiled-ws")
-    g.init_fields(d["rho"], d["ux"], d["uy"], d["uz"], d["phi"], d["pineq"])
-    g.step(10)
-    m = {k: (None if v is None else np.asarray(v, dtype=np.float64)) for k, v in g.get_moments().items()}
-    for k, v in errs(m, r).items():
-        assert v <= 1e-5, (k, v)
-    g.close()
-    jp = inputs.jet_params(64, 64, 24, D=10, U=0.05, Re=500.0, We=100.0, perturbation=0.05, seed=3)
-    d, r = oracle_run("ws-jet", lambda: inputs.jet_developed(64, 64, 24, D=10, ndrop=6), jp, 10, tslb.F32)
-    g = tslb.Tslb(64, 64, 24, jp["omega"], precision=tslb.F32, kernel=tslb.KERNEL_TILED, **gpu_kwargs(jp))
-    g.init_fields(d["rho"], d["ux"], d["uy"], d["uz"], d["phi"])
-    g.step(10)
-    m = {k: (None if v is None else np.asarray(v, dtype=np.float64)) for k, v in g.get_moments().items()}
-    for k, v in errs(m, r).items():
-        assert v <= 1e-5, (k, v)
-    g.close()
