@@ -107,7 +107,6 @@ struct TileCfg {
   static constexpr int GQE = RY * TX;      // region rows x tile columns
   static constexpr int FQE = RY * FQW;     // one scalar per node pair
   static constexpr int TLE = TY * TX;      // tile nodes
-  static constexpr int XHE = 2 * 8 * RY;   // [2 sides][8 groups][RY]
   static constexpr int B_ZC = 0;                                 // [3]  D_x S_z n_x, S_x S_z n_y, S_x d_z n_z
   static constexpr int B_ZL = B_ZC + (TWO ? 3 * ZCE : 0);        // [3]  S_z n_x, S_z n_y, d_z n_z on the halo columns
   static constexpr int B_ZZ = B_ZL + (TWO ? 3 * ZLE : 0);        // [3]  zeros (what the lanes off the tile edge read)
@@ -116,10 +115,13 @@ struct TileCfg {
   static constexpr int B_KF = B_FQ + (TWO ? 2 * FQE : 0);        // [3]  F = sigma kappa grad(phi), phase -> flow
   static constexpr int B_GR = B_KF + (TWO ? 3 * TLE : 0);        // [3]  grad(phi), private to the owning phase thread
   static constexpr int B_PH = B_GR + (TWO ? 3 * TLE : 0);        // [1]  own phi, private to the owning phase thread
-  static constexpr int B_XH = B_PH + (TWO ? TLE : 0);            // x-pass terms of the two halo columns
-  static constexpr int BUF = (B_XH + XHE + 3) / 4 * 4;           // elements per half
+  static constexpr int BUF = (B_PH + (TWO ? TLE : 0) + 3) / 4 * 4;   // elements per half
   static_assert(ZCE % 2 == 0 && ZLE % 2 == 0 && GQE % 2 == 0 && FQE % 2 == 0, "pair alignment");
-  static constexpr int YPF = TY * TX;      // y-push field: TY sending rows
+  // y-push field: TY sending rows, and one more row that holds the x-pass terms of a halo column for the
+  // lanes at the tile edge ([2 plane parities][RY]; a+ of column x0-1 in the a+ fields, a- of column
+  // x0+TX in the a- fields), so that they sit at the same field stride as the lanes' own x-exchange words
+  static constexpr int YPF = (TY + 1) * TX;
+  static_assert(2 * RY <= TX, "halo-column terms fit one row");
   static constexpr size_t OFF_MOM = 0;
   static constexpr size_t OFF_PHI = OFF_MOM + S * MOM_STAGE;
   static constexpr size_t OFF_BUF = OFF_PHI + (TWO ? S * PHI_STAGE : 0);    // [2][BUF]
@@ -223,13 +225,13 @@ struct PairGeom {
 // through its peer pointers (phi from the two planes next to the face, the moments from the face
 // plane).  The field arrays of a buffer are equally spaced (fs elements).
 template <typename T, unsigned MASK, bool SLAB>
-__device__ __forceinline__ void store_pair(const StepParams<T> &P, const Pair<T> *o, int j, long long o00, int gx, int gy,
-                                           bool edge, long long fs) {
+__device__ __forceinline__ void store_pair(const StepParams<T> &P, const Pair<T> *o, T *p0, int j, int gx, int gy, bool edge,
+                                           long long fs) {
+  // p0: field 0 at this node pair and plane
   typedef Pair<T> V;
   const Layout &L = P.L;
-  const long long zo = (long long)j * L.plane;
   {
-    T *p = P.out.f[0] + zo + o00;
+    T *p = p0;
     int last = 0;
 #pragma unroll
     for (int m = 0; m < NF_MAX; ++m)
@@ -237,9 +239,10 @@ __device__ __forceinline__ void store_pair(const StepParams<T> &P, const Pair<T>
   }
   const bool push = SLAB && ((j < 2 && P.nb[0].f[0]) || (j >= L.nz - 2 && P.nb[1].f[0]));
   if (edge || push) {
+    const long long zo = (long long)j * L.plane;
     const int gxg = gx < 2 ? gx + L.nx : (gx >= L.nx - 2 ? gx - L.nx : gx);
     const int gyg = gy < GY ? gy + L.ny : (gy >= L.ny - GY ? gy - L.ny : gy);
-    const long long o10 = L.idx(gxg, gy, 0), o01 = L.idx(gx, gyg, 0), o11 = L.idx(gxg, gyg, 0);
+    const long long o00 = L.idx(gx, gy, 0), o10 = L.idx(gxg, gy, 0), o01 = L.idx(gx, gyg, 0), o11 = L.idx(gxg, gyg, 0);
     if (gxg != gx || gyg != gy) {
 #pragma unroll 1
       for (int im = 0; im < 3; ++im) {       // one copy of the store code: x image, y image, corner
@@ -368,6 +371,12 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   const long long o00 = L.idx(gx_, gy_, 0);
   const bool edge_tile = x0 == 0 || x0 + TX == L.nx || y0 < GY || y0 + TY > L.ny - GY;
 
+  // planes whose phi' a tile pair stores (rows r and r + 2 of a phase thread): its chunk, without the imposed
+  // inflow / outflow planes; nothing when the node belongs to the neighbouring (shifted-back) tile
+  const int pjlo = max(z0, P.jet_lo ? 1 : 0);
+  const int pnj = min(z1, P.out_hi ? L.nz - 1 : L.nz) - pjlo;
+  const int pnjs0 = (gx_ >= xs && gy_ >= ys) ? pnj : 0, pnjs1 = (gx_ >= xs && gy_ + 2 >= ys) ? pnj : 0;
+
   // B: phase geometry and fluxes of one node pair (eqs. 20-24, readings A6-A8), iteration k.
   // ROLE 0: a tile pair (finishes and stores phi'); 1: a halo-row pair; 2: a halo-column pair.
   // bo / bn: element offsets of the exchange-block halves of plane parity k&1 / (k-1)&1.
@@ -452,8 +461,9 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
       V o[NF_MAX];
       o[F_PHI] = pfma((xin + yin) + (ph - qz), T(0.125), st.acc);
       const int j = k - 1;
-      if (j >= z0 && j < z1 && gx_ >= xs && gy_ + DR >= ys && !((P.jet_lo && j == 0) || (P.out_hi && j == L.nz - 1)))
-        store_pair<T, FM_PHI, SLAB>(P, o, j, o00 + (long long)DR * L.px, gx_, gy_ + DR, edge_tile, fs);
+      if ((unsigned)(j - pjlo) < (unsigned)(DR ? pnjs1 : pnjs0))
+        store_pair<T, FM_PHI, SLAB>(P, o, P.out.f[0] + ((long long)j * L.plane + o00 + (long long)DR * L.px), j, gx_, gy_ + DR,
+                                    edge_tile, fs);
       st.acc = pfma(V(fm.y, fp.x) + st.cup, T(0.125), ph * T(0.25));
       st.cup = ph + qz;
     }
@@ -494,74 +504,94 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     s = s == S - 1 ? 0 : s + 1;
     if (s == 0) mph ^= 1u;
   };
+  // Register file: 2 CTAs x 8 warps leave 128 registers per thread; the flow warps (one warp group) need
+  // more, the other warp group less.
+  constexpr bool REGSPLIT = false && TWO && C::CTAS_PER_SM == 2 && C::NWF == 4;
 
-  if (flow || halow) {
-    // ============================ flow warps and the halo-row warp ============================
+  // A: x-pass of region row r of plane k in push form, then the y-push terms (flow warps and the halo-row
+  // warp).  Each node's K is evaluated once; a+ / a- cross to the x-neighbour thread through shared memory
+  // (same warp); the lanes at the tile edge take the halo column's term, which the halo-column warp left in
+  // the extra row of the same fields one iteration earlier.
+  const bool st_ap = r <= TY - 1, st_am = r >= 2;        // rows 0..TY-1 send an a+, rows 2..TY+1 an a-
+  auto xpass = [&](int k, int s, V (&A0)[9]) {
+    // y-push fields: a+ is stored at row index r, a- at r-2; a tile row r reads both at index r-1 (= oT)
+    const int oAP = r * TX + 2 * lx, oAM = oAP - 2 * TX;
+    // x-exchange word of this lane: word `lane` of a row of the y-push fields 0..7 that this warp is about
+    // to overwrite (a+ field: the warp's first sending row; a- field: its last)
+    T *const xp = s_ap + (flow ? 2 * wid + 1 : 0) * TX + lane, *const xm = s_am + (flow ? 2 * wid : TY - 1) * TX + lane;
+    const int hrow = TY * TX + (k & 1) * RY + r;         // the halo-column terms of plane k, row r
+    const T *pl = lx == 0 ? s_ap + hrow : xp - 1, *pr = lx == LX - 1 ? s_am + hrow : xm + 1;
+    V Xg[8][3];   // [group][p]
+    {
+      V m[10], K[NK];
+      const T *p = mom_at(s) + oM;
+#pragma unroll
+      for (int f = 0; f < 10; ++f) m[f] = lds_pair(p + f * MF);
+      hermite_coeffs<ORDER, V>(m[0], m[1], m[2], m[3], m[4], m[5], m[6], m[7], m[8], m[9], omc, K);
+      V gp[8], gm[8], g0[8];
+      push3<3, V, T>(K[K000], K[K100], K[K200], gp[0], gm[0], g0[0]);   // (b,c) = (0,0)
+      push3<3, V, T>(K[K010], K[K110], K[K210], gp[1], gm[1], g0[1]);   // (1,0)
+      push3<2, V, T>(K[K020], K[K120], K[K120], gp[2], gm[2], g0[2]);   // (2,0)
+      push3<3, V, T>(K[K001], K[K101], K[K201], gp[3], gm[3], g0[3]);   // (0,1)
+      push3<2, V, T>(K[K011], K[K111], K[K111], gp[4], gm[4], g0[4]);   // (1,1)
+      push3<1, V, T>(K[K021], K[K021], K[K021], gp[5], gm[5], g0[5]);   // (2,1)
+      push3<2, V, T>(K[K002], K[K102], K[K102], gp[6], gm[6], g0[6]);   // (0,2)
+      push3<1, V, T>(K[K012], K[K012], K[K012], gp[7], gm[7], g0[7]);   // (1,2)
+      // lane l of the warp parks gp.y / gm.x at word l of one of the warp's own y-push rows
+#pragma unroll
+      for (int g = 0; g < 8; ++g) { xp[g * YPF] = gp[g].y; xm[g * YPF] = gm[g].x; }
+      __syncwarp();
+#pragma unroll
+      for (int g = 0; g < 8; ++g) {
+        pull3s<V, T>(pl[g * YPF], gp[g].x, gm[g].y, pr[g * YPF], g0[g], Xg[g][0], Xg[g][1], Xg[g][2]);
+      }
+      __syncwarp();
+    }
+    // y-push per (c, p): groups of c = 0: b = 0,1,2 -> g 0,1,2; c = 1: g 3,4,5; c = 2: b = 0,1 -> g 6,7
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+      for (int p = 0; p < 3; ++p) {
+        V ap, am;
+        if (c < 2) push3<3, V, T>(Xg[3 * c][p], Xg[3 * c + 1][p], Xg[3 * c + 2][p], ap, am, A0[3 * c + p]);
+        else push3<2, V, T>(Xg[6][p], Xg[7][p], Xg[7][p], ap, am, A0[6 + p]);
+        sts_pair_if(st_ap, s_ap + (3 * c + p) * YPF + oAP, ap);
+        sts_pair_if(st_am, s_am + (3 * c + p) * YPF + oAM, am);
+      }
+  };
+  // the y-push terms of a plane are complete: a barrier among the flow warps and the halo-row warp only
+  auto xpass_barrier = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(C::NXPASS) : "memory"); };
+
+  if (flow) {
+    // ============================ flow warps ============================
+    if (REGSPLIT) asm volatile("setmaxnreg.inc.sync.aligned.u32 152;");
     V accA[10], accB[10];     // Hermite moments being accumulated for planes k and k+1
     V ubx(T(0)), uby(T(0)), ubz(T(0)), rinv(T(1));   // u_b and 1/rho' of the plane completed last
 #pragma unroll
     for (int m = 0; m < 10; ++m) { accA[m] = V(T(0)); accB[m] = V(T(0)); }
-    // y-push fields: a+ is stored at row index r (rows 0..TY-1 send one), a- at r-2 (rows 2..TY+1);
-    // a tile row r reads both at index r-1 (= oT)
-    const bool st_ap = r <= TY - 1, st_am = r >= 2;
-    const int oAP = r * TX + 2 * lx, oAM = oAP - 2 * TX;
-    // x-exchange word of this lane: word `lane` of a row of the y-push fields 0..7 that this warp is
-    // about to overwrite (a+ field: the warp's first sending row; a- field: its last)
-    T *const xp = s_ap + (flow ? 2 * wid + 1 : 0) * TX + lane, *const xm = s_am + (flow ? 2 * wid : TY - 1) * TX + lane;
+    // planes this thread stores: its chunk, without the imposed inflow / outflow planes; nothing when the
+    // node belongs to the neighbouring (shifted-back) tile
+    const int jlo = max(z0, P.jet_lo ? 1 : 0);
+    const int njs = (gx_ >= xs && gy_ >= ys) ? min(z1, P.out_hi ? L.nz - 1 : L.nz) - jlo : 0;
+    T *pst = P.out.f[0] + o00 + (long long)(kst - 2) * L.plane;   // field 0 of the pair, plane k-2
     for (int i = 0; i < NI; ++i) {
       const int k = kst + i;
       const int bo = (k & 1) * BUF;          // exchange-block half of this plane's parity
       if (has_group(k)) mbar_wait(&bars[s], mph);
       const bool src = k >= z0 - 1 && k <= z1;     // plane k is a source plane of this chunk
       V A0[9];                               // own y-push term a0 per (c,p)
-      if (src) {
-        // A: x-pass of region row r of plane k in push form, then the y-push terms.  Each node's K is
-        // evaluated once; a+ / a- cross to the x-neighbour thread through shared memory (same warp).
-        const T *xh = s_buf + bo + C::B_XH;
-        V Xg[8][3];   // [group][p]
-        {
-          V m[10], K[NK];
-          const T *p = mom_at(s) + oM;
-#pragma unroll
-          for (int f = 0; f < 10; ++f) m[f] = lds_pair(p + f * MF);
-          hermite_coeffs<ORDER, V>(m[0], m[1], m[2], m[3], m[4], m[5], m[6], m[7], m[8], m[9], omc, K);
-          V gp[8], gm[8], g0[8];
-          push3<3, V, T>(K[K000], K[K100], K[K200], gp[0], gm[0], g0[0]);   // (b,c) = (0,0)
-          push3<3, V, T>(K[K010], K[K110], K[K210], gp[1], gm[1], g0[1]);   // (1,0)
-          push3<2, V, T>(K[K020], K[K120], K[K120], gp[2], gm[2], g0[2]);   // (2,0)
-          push3<3, V, T>(K[K001], K[K101], K[K201], gp[3], gm[3], g0[3]);   // (0,1)
-          push3<2, V, T>(K[K011], K[K111], K[K111], gp[4], gm[4], g0[4]);   // (1,1)
-          push3<1, V, T>(K[K021], K[K021], K[K021], gp[5], gm[5], g0[5]);   // (2,1)
-          push3<2, V, T>(K[K002], K[K102], K[K102], gp[6], gm[6], g0[6]);   // (0,2)
-          push3<1, V, T>(K[K012], K[K012], K[K012], gp[7], gm[7], g0[7]);   // (1,2)
-          // lane l of the warp parks gp.y / gm.x at word l of one of the warp's own y-push rows
-#pragma unroll
-          for (int g = 0; g < 8; ++g) { xp[g * YPF] = gp[g].y; xm[g * YPF] = gm[g].x; }
-          __syncwarp();
-          // left / right neighbour's word, or the halo column's term for the lanes at the tile edge
-          const T *pl = lx == 0 ? xh + r : xp - 1, *pr = lx == LX - 1 ? xh + 8 * RY + r : xm + 1;
-          const int sl = lx == 0 ? RY : YPF, sr = lx == LX - 1 ? RY : YPF;
-#pragma unroll
-          for (int g = 0; g < 8; ++g) {
-            pull3s<V, T>(pl[g * sl], gp[g].x, gm[g].y, pr[g * sr], g0[g], Xg[g][0], Xg[g][1], Xg[g][2]);
-          }
-          __syncwarp();
-        }
-        // y-push per (c, p): groups of c = 0: b = 0,1,2 -> g 0,1,2; c = 1: g 3,4,5; c = 2: b = 0,1 -> g 6,7
-#pragma unroll
-        for (int c = 0; c < 3; ++c)
-#pragma unroll
-          for (int p = 0; p < 3; ++p) {
-            V ap, am;
-            if (c < 2) push3<3, V, T>(Xg[3 * c][p], Xg[3 * c + 1][p], Xg[3 * c + 2][p], ap, am, A0[3 * c + p]);
-            else push3<2, V, T>(Xg[6][p], Xg[7][p], Xg[7][p], ap, am, A0[6 + p]);
-            sts_pair_if(st_ap, s_ap + (3 * c + p) * YPF + oAP, ap);
-            sts_pair_if(st_am, s_am + (3 * c + p) * YPF + oAM, am);
-          }
+      if (src) xpass(k, s, A0);
+      xpass_barrier();
+      V o[NF_MAX];
+      if (TWO && (unsigned)(k - 2 - jlo) < (unsigned)njs) {
+        // a6: u'(k-2) = u_b + F / rho' with the F(k-2) the phase warps wrote in iteration k-1; a9: store it
+        const T *kf = s_buf + bo + C::B_KF + oT;
+        o[1] = pfma(lds_pair(kf), rinv, ubx);
+        o[2] = pfma(lds_pair(kf + TLE), rinv, uby);
+        o[3] = pfma(lds_pair(kf + 2 * TLE), rinv, ubz);
+        store_pair<T, FM_U, SLAB>(P, o, pst, k - 2, gx_, gy_, edge_tile, fs);
       }
-      // the y-push terms of plane k are complete (flow warps and the halo-row warp only)
-      asm volatile("bar.sync 1, %0;" ::"n"(C::NXPASS) : "memory");
-      if (flow && src) {
+      if (src) {
         // C: finish the y-pass of plane k (a+ from the row below, a- from the row above, own a0) and z-push
         const T *yu = s_ap + oT, *yd = s_am + oT;
         V outm[10];
@@ -596,24 +626,10 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
             }
           }
         }
-        const bool mine = gx_ >= xs && gy_ >= ys;
-        V o[NF_MAX];
-        if (TWO) {
-          // a6: u'(k-2) = u_b + F / rho' with the F(k-2) of the phase warps; a9: store it
-          const int j = k - 2;
-          if (j >= z0 && mine && !((P.jet_lo && j == 0) || (P.out_hi && j == L.nz - 1))) {
-            const T *kf = s_buf + bo + C::B_KF + oT;
-            o[1] = pfma(lds_pair(kf), rinv, ubx);
-            o[2] = pfma(lds_pair(kf + TLE), rinv, uby);
-            o[3] = pfma(lds_pair(kf + 2 * TLE), rinv, ubz);
-            store_pair<T, FM_U, SLAB>(P, o, j, o00, gx_, gy_, edge_tile, fs);
-          }
-        }
         // a4: plane k-1 is complete: u_b = m'/rho', Pi^neq' = Pi' - rho' u_b u_b (Hermite form)
         rinv = prcp<T>(outm[0] + V(T(1)));
         ubx = outm[1] * rinv; uby = outm[2] * rinv; ubz = outm[3] * rinv;
-        const int j = k - 1;
-        if (j >= z0 && mine && !((P.jet_lo && j == 0) || (P.out_hi && j == L.nz - 1))) {
+        if ((unsigned)(k - 1 - jlo) < (unsigned)njs) {
           o[0] = outm[0];
           o[4] = outm[4] - outm[1] * ubx;
           o[5] = outm[5] - outm[2] * uby;
@@ -622,28 +638,30 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
           o[8] = outm[8] - outm[1] * ubz;
           o[9] = outm[9] - outm[2] * ubz;
           if (TWO) {
-            store_pair<T, FM_RHOPI, SLAB>(P, o, j, o00, gx_, gy_, edge_tile, fs);
+            store_pair<T, FM_RHOPI, SLAB>(P, o, pst + L.plane, k - 1, gx_, gy_, edge_tile, fs);
           } else {
             o[1] = ubx; o[2] = uby; o[3] = ubz;
-            store_pair<T, FM_FLOW, SLAB>(P, o, j, o00, gx_, gy_, edge_tile, fs);
+            store_pair<T, FM_FLOW, SLAB>(P, o, pst + L.plane, k - 1, gx_, gy_, edge_tile, fs);
           }
         }
-      } else if (TWO && flow && k == z1 + 1) {
-        // the kick and the velocity of the chunk's last plane
-        const int j = k - 2;
-        if (gx_ >= xs && gy_ >= ys && !((P.jet_lo && j == 0) || (P.out_hi && j == L.nz - 1))) {
-          V o[NF_MAX];
-          const T *kf = s_buf + bo + C::B_KF + oT;
-          o[1] = pfma(lds_pair(kf), rinv, ubx);
-          o[2] = pfma(lds_pair(kf + TLE), rinv, uby);
-          o[3] = pfma(lds_pair(kf + 2 * TLE), rinv, ubz);
-          store_pair<T, FM_U, SLAB>(P, o, j, o00, gx_, gy_, edge_tile, fs);
-        }
       }
+      pst += L.plane;
+      iter_end(k);
+    }
+  } else if (halow) {
+    // ============================ halo-row warp ============================
+    if (REGSPLIT) asm volatile("setmaxnreg.dec.sync.aligned.u32 104;");
+    for (int i = 0; i < NI; ++i) {
+      const int k = kst + i;
+      if (has_group(k)) mbar_wait(&bars[s], mph);
+      V A0[9];
+      if (k >= z0 - 1 && k <= z1) xpass(k, s, A0);
+      xpass_barrier();
       iter_end(k);
     }
   } else if (colw) {
     // ============================ halo-column warp ============================
+    if (REGSPLIT) asm volatile("setmaxnreg.dec.sync.aligned.u32 104;");
     // node pairs: lanes 0 .. 2 RY - 1 own the two halo columns; every lane owns a pair of the halo rows
     PhaseState<T> pc, ph_;
     pc.clear(); ph_.clear();
@@ -675,9 +693,9 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
           push3<1, T, T>(K[K021], K[K021], K[K021], gp[5], gm[5], g0);
           push3<2, T, T>(K[K002], K[K102], K[K102], gp[6], gm[6], g0);
           push3<1, T, T>(K[K012], K[K012], K[K012], gp[7], gm[7], g0);
-          T *xh = s_buf + bn + C::B_XH + cside * 8 * RY + r;
+          T *xh = (cside ? s_am : s_ap) + TY * TX + ((k + 1) & 1) * RY + r;
 #pragma unroll
-          for (int g = 0; g < 8; ++g) xh[g * RY] = cside ? gm[g] : gp[g];
+          for (int g = 0; g < 8; ++g) xh[g * YPF] = cside ? gm[g] : gp[g];
         }
       }
       if (TWO && k <= z1) {
@@ -688,6 +706,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     }
   } else {
     // ============================ phase warps ============================
+    if (REGSPLIT) asm volatile("setmaxnreg.dec.sync.aligned.u32 104;");
     PhaseState<T> p0, p1;     // two node pairs: rows r and r + 2
     p0.clear(); p1.clear();
     const int oZ = r * ZW + 2 + 2 * lx, oF = r * FQW + 1 + lx, oG = r * TX + 2 * lx;
