@@ -220,30 +220,21 @@ struct PairGeom {
   int oP, c0, cl, cr, oZ, oF, oG, oT;
 };
 
-// Store the fields of MASK (bit m = field m) of one node pair of plane j: the node itself, its periodic
-// ghost images (edge tiles only) and, on a slab face, the same into the neighbour slab's ghost planes
-// through its peer pointers (phi from the two planes next to the face, the moments from the face
-// plane).  The field arrays of a buffer are equally spaced (fs elements).
+// The rare part of a store of the fields of MASK (bit m = field m) of one node pair of plane j at (gx, gy):
+// its periodic ghost images (nodes next to the domain edge) and, on a slab face, the same values into the
+// neighbour slab's ghost planes through its peer pointers (phi from the two planes next to the face, the
+// moments from the face plane).  img: the pair has a ghost image.
 template <typename T, unsigned MASK, bool SLAB>
-__device__ __forceinline__ void store_pair(const StepParams<T> &P, const Pair<T> *o, T *p0, int j, int gx, int gy, bool edge,
-                                           long long fs) {
-  // p0: field 0 at this node pair and plane
+__device__ __forceinline__ void store_rare(const StepParams<T> &P, const Pair<T> *o, int j, int gx, int gy, bool img) {
   typedef Pair<T> V;
   const Layout &L = P.L;
-  {
-    T *p = p0;
-    int last = 0;
-#pragma unroll
-    for (int m = 0; m < NF_MAX; ++m)
-      if (MASK >> m & 1u) { p += (m - last) * fs; last = m; *reinterpret_cast<V *>(p) = o[m]; }
-  }
   const bool push = SLAB && ((j < 2 && P.nb[0].f[0]) || (j >= L.nz - 2 && P.nb[1].f[0]));
-  if (edge || push) {
+  if (img || push) {
     const long long zo = (long long)j * L.plane;
     const int gxg = gx < 2 ? gx + L.nx : (gx >= L.nx - 2 ? gx - L.nx : gx);
     const int gyg = gy < GY ? gy + L.ny : (gy >= L.ny - GY ? gy - L.ny : gy);
     const long long o00 = L.idx(gx, gy, 0), o10 = L.idx(gxg, gy, 0), o01 = L.idx(gx, gyg, 0), o11 = L.idx(gxg, gyg, 0);
-    if (gxg != gx || gyg != gy) {
+    if (img) {
 #pragma unroll 1
       for (int im = 0; im < 3; ++im) {       // one copy of the store code: x image, y image, corner
         if (im == 0 ? gxg == gx : (im == 1 ? gyg == gy : (gxg == gx || gyg == gy))) continue;
@@ -270,6 +261,27 @@ __device__ __forceinline__ void store_pair(const StepParams<T> &P, const Pair<T>
       }
     }
   }
+}
+// Store the fields of MASK (bit m = field m) of one node pair of plane j.  p0: field 0 at this pair and
+// plane; the field arrays of a buffer are equally spaced (fs elements).
+template <typename T, unsigned MASK, bool SLAB>
+__device__ __forceinline__ void store_pair(const StepParams<T> &P, const Pair<T> *o, T *p0, int j, int gx, int gy, bool img,
+                                           long long fs) {
+  T *p = p0;
+  int last = 0;
+#pragma unroll
+  for (int m = 0; m < NF_MAX; ++m)
+    if (MASK >> m & 1u) { p += (m - last) * fs; last = m; *reinterpret_cast<Pair<T> *>(p) = o[m]; }
+  store_rare<T, MASK, SLAB>(P, o, j, gx, gy, img);
+}
+// predicated global pair store (one instruction, no branch)
+__device__ __forceinline__ void stg_pair_if(bool p, float *a, Pair<float> v) {
+  asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %0, 0;\n@q st.global.v2.f32 [%1], {%2, %3};\n}"
+               ::"r"((int)p), "l"(a), "f"(v.x), "f"(v.y) : "memory");
+}
+__device__ __forceinline__ void stg_pair_if(bool p, double *a, Pair<double> v) {
+  asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %0, 0;\n@q st.global.v2.f64 [%1], {%2, %3};\n}"
+               ::"r"((int)p), "l"(a), "d"(v.x), "d"(v.y) : "memory");
 }
 constexpr unsigned FM_U = 0xEu, FM_RHOPI = 0x3F1u, FM_FLOW = 0x3FFu, FM_PHI = 0x400u;   // field masks
 
@@ -369,13 +381,9 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   // global coordinates / store offset (plane 0) of the thread's (first) pair
   const int gx_ = x0 + 2 * lx, gy_ = y0 + r - 1;
   const long long o00 = L.idx(gx_, gy_, 0);
-  const bool edge_tile = x0 == 0 || x0 + TX == L.nx || y0 < GY || y0 + TY > L.ny - GY;
-
-  // planes whose phi' a tile pair stores (rows r and r + 2 of a phase thread): its chunk, without the imposed
-  // inflow / outflow planes; nothing when the node belongs to the neighbouring (shifted-back) tile
-  const int pjlo = max(z0, P.jet_lo ? 1 : 0);
-  const int pnj = min(z1, P.out_hi ? L.nz - 1 : L.nz) - pjlo;
-  const int pnjs0 = (gx_ >= xs && gy_ >= ys) ? pnj : 0, pnjs1 = (gx_ >= xs && gy_ + 2 >= ys) ? pnj : 0;
+  // the pair (and, for a phase thread, its second pair two rows up) has a periodic ghost image
+  const bool imgx = gx_ < 2 || gx_ >= L.nx - 2;
+  const bool img0 = imgx || gy_ < GY || gy_ >= L.ny - GY, img1 = imgx || gy_ + 2 < GY || gy_ + 2 >= L.ny - GY;
 
   // B: phase geometry and fluxes of one node pair (eqs. 20-24, readings A6-A8), iteration k.
   // ROLE 0: a tile pair (finishes and stores phi'); 1: a halo-row pair; 2: a halo-column pair.
@@ -425,6 +433,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     // a7 in push form: the node sends phi + q_a along +e_a and phi - q_a along -e_a,
     // q_a = phi (4 u_a + gamma (1 - phi) n_a), of plane k
     const T *mo = mom_at(s) + g.oP + g.c0;
+    V phinew(T(0));                                                     // phi'(k-1) (tile pairs)
     V ph;                                                               // own phi(k)
     if (ROLE == 0) {
       // tile pairs keep their own phi(k), phi(k+1) in a private two-slot ring (slot = plane parity)
@@ -453,21 +462,17 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
       // grad(phi) of plane k+1 for the kick two iterations on: private two-slot ring (slot = plane parity)
       T *gr_ = s_buf + bn + C::B_GR + g.oT;
       sts_pair(gr_, gx); sts_pair(gr_ + TLE, gy); sts_pair(gr_ + 2 * TLE, gz);
-      // phi'(k-1) = phi/4 + (in-plane arrivals of plane k-1 + up(k-2) + down(k)) / 8, stored at once
+      // phi'(k-1) = phi/4 + (in-plane arrivals of plane k-1 + up(k-2) + down(k)) / 8
       const T *fr = s_buf + bn + C::B_FQ + g.oF;
       const T *gr = s_buf + bn + C::B_GQ + g.oG;
       const V xin(fr[-1], fr[FQE + 1]);
       const V yin = lds_pair(gr - TX) + lds_pair(gr + GQE + TX);
-      V o[NF_MAX];
-      o[F_PHI] = pfma((xin + yin) + (ph - qz), T(0.125), st.acc);
-      const int j = k - 1;
-      if ((unsigned)(j - pjlo) < (unsigned)(DR ? pnjs1 : pnjs0))
-        store_pair<T, FM_PHI, SLAB>(P, o, P.out.f[0] + ((long long)j * L.plane + o00 + (long long)DR * L.px), j, gx_, gy_ + DR,
-                                    edge_tile, fs);
+      phinew = pfma((xin + yin) + (ph - qz), T(0.125), st.acc);
       st.acc = pfma(V(fm.y, fp.x) + st.cup, T(0.125), ph * T(0.25));
       st.cup = ph + qz;
     }
     st.DZ = st.nB[2] * T(-0.5); st.nB[2] = nCz;
+    return phinew;
   };
 
   // D: kappa(k-1) = -(S_y ax + D_y bx + S_y cx) from the x-combined z-combinations of n written in iteration
@@ -497,16 +502,14 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   // ring slot of this iteration's group (group kfirst sits in slot 0) and its mbarrier phase parity
   int s = TWO ? 0 : S - 1;
   uint32_t mph = TWO ? 0u : 1u;
-  // end of an iteration: the ONE CTA barrier; the group three planes ahead goes into the slot just read
-  auto iter_end = [&](int k) {
+  // end of an iteration: the ONE CTA barrier; in the halo-column warp (ISSUE) the group three planes ahead
+  // goes into the slot just read
+  auto iter_end = [&](auto issues, int k) {
     __syncthreads();
-    if (issuer && k >= kfirst && has_group(k + S)) issue(k + S, s);
+    if (decltype(issues)::value && issuer && k >= kfirst && has_group(k + S)) issue(k + S, s);
     s = s == S - 1 ? 0 : s + 1;
     if (s == 0) mph ^= 1u;
   };
-  // Register file: 2 CTAs x 8 warps leave 128 registers per thread; the flow warps (one warp group) need
-  // more, the other warp group less.
-  constexpr bool REGSPLIT = false && TWO && C::CTAS_PER_SM == 2 && C::NWF == 4;
 
   // A: x-pass of region row r of plane k in push form, then the y-push terms (flow warps and the halo-row
   // warp).  Each node's K is evaluated once; a+ / a- cross to the x-neighbour thread through shared memory
@@ -562,9 +565,8 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   // the y-push terms of a plane are complete: a barrier among the flow warps and the halo-row warp only
   auto xpass_barrier = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(C::NXPASS) : "memory"); };
 
-  if (flow) {
-    // ============================ flow warps ============================
-    if (REGSPLIT) asm volatile("setmaxnreg.inc.sync.aligned.u32 152;");
+  if (flow || halow) {
+    // ============================ flow warps and the halo-row warp ============================
     V accA[10], accB[10];     // Hermite moments being accumulated for planes k and k+1
     V ubx(T(0)), uby(T(0)), ubz(T(0)), rinv(T(1));   // u_b and 1/rho' of the plane completed last
 #pragma unroll
@@ -583,15 +585,15 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
       if (src) xpass(k, s, A0);
       xpass_barrier();
       V o[NF_MAX];
-      if (TWO && (unsigned)(k - 2 - jlo) < (unsigned)njs) {
+      if (TWO && flow && (unsigned)(k - 2 - jlo) < (unsigned)njs) {
         // a6: u'(k-2) = u_b + F / rho' with the F(k-2) the phase warps wrote in iteration k-1; a9: store it
         const T *kf = s_buf + bo + C::B_KF + oT;
         o[1] = pfma(lds_pair(kf), rinv, ubx);
         o[2] = pfma(lds_pair(kf + TLE), rinv, uby);
         o[3] = pfma(lds_pair(kf + 2 * TLE), rinv, ubz);
-        store_pair<T, FM_U, SLAB>(P, o, pst, k - 2, gx_, gy_, edge_tile, fs);
+        store_pair<T, FM_U, SLAB>(P, o, pst, k - 2, gx_, gy_, img0, fs);
       }
-      if (src) {
+      if (flow && src) {
         // C: finish the y-pass of plane k (a+ from the row below, a- from the row above, own a0) and z-push
         const T *yu = s_ap + oT, *yd = s_am + oT;
         V outm[10];
@@ -638,30 +640,18 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
           o[8] = outm[8] - outm[1] * ubz;
           o[9] = outm[9] - outm[2] * ubz;
           if (TWO) {
-            store_pair<T, FM_RHOPI, SLAB>(P, o, pst + L.plane, k - 1, gx_, gy_, edge_tile, fs);
+            store_pair<T, FM_RHOPI, SLAB>(P, o, pst + L.plane, k - 1, gx_, gy_, img0, fs);
           } else {
             o[1] = ubx; o[2] = uby; o[3] = ubz;
-            store_pair<T, FM_FLOW, SLAB>(P, o, pst + L.plane, k - 1, gx_, gy_, edge_tile, fs);
+            store_pair<T, FM_FLOW, SLAB>(P, o, pst + L.plane, k - 1, gx_, gy_, img0, fs);
           }
         }
       }
       pst += L.plane;
-      iter_end(k);
-    }
-  } else if (halow) {
-    // ============================ halo-row warp ============================
-    if (REGSPLIT) asm volatile("setmaxnreg.dec.sync.aligned.u32 104;");
-    for (int i = 0; i < NI; ++i) {
-      const int k = kst + i;
-      if (has_group(k)) mbar_wait(&bars[s], mph);
-      V A0[9];
-      if (k >= z0 - 1 && k <= z1) xpass(k, s, A0);
-      xpass_barrier();
-      iter_end(k);
+      iter_end(IC<0>(), k);
     }
   } else if (colw) {
     // ============================ halo-column warp ============================
-    if (REGSPLIT) asm volatile("setmaxnreg.dec.sync.aligned.u32 104;");
     // node pairs: lanes 0 .. 2 RY - 1 own the two halo columns; every lane owns a pair of the halo rows
     PhaseState<T> pc, ph_;
     pc.clear(); ph_.clear();
@@ -702,11 +692,10 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
         if (lane < 2 * RY) phase_B(IC<2>(), IC<0>(), pc, gc, k, s, bo, bn);
         phase_B(IC<1>(), IC<0>(), ph_, gh, k, s, bo, bn);
       }
-      iter_end(k);
+      iter_end(IC<1>(), k);
     }
   } else {
     // ============================ phase warps ============================
-    if (REGSPLIT) asm volatile("setmaxnreg.dec.sync.aligned.u32 104;");
     PhaseState<T> p0, p1;     // two node pairs: rows r and r + 2
     p0.clear(); p1.clear();
     const int oZ = r * ZW + 2 + 2 * lx, oF = r * FQW + 1 + lx, oG = r * TX + 2 * lx;
@@ -716,16 +705,32 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     const int eoff = (lx == 0 ? C::B_ZL : (lx == LX - 1 ? C::B_ZL + RY : C::B_ZZ)) + 2 + r;
     const V emask(lx == 0 ? T(1) : T(0), lx == LX - 1 ? T(1) : T(0));
     const T esign = lx == 0 ? T(-0.5) : T(0.5);
+    // planes whose phi' the thread stores (rows r and r + 2): its chunk, without the imposed inflow / outflow
+    // planes; nothing when the node belongs to the neighbouring (shifted-back) tile
+    const int pjlo = max(z0, P.jet_lo ? 1 : 0);
+    const int pnj = min(z1, P.out_hi ? L.nz - 1 : L.nz) - pjlo;
+    const int pnjs0 = (gx_ >= xs && gy_ >= ys) ? pnj : 0, pnjs1 = (gx_ >= xs && gy_ + 2 >= ys) ? pnj : 0;
+    T *pph = P.out.f[F_PHI] + o00 + (long long)(kst - 1) * L.plane;   // phi of the first pair, plane k-1
     for (int i = 0; i < NI; ++i) {
       const int k = kst + i;
       const int bo = (k & 1) * BUF, bn = BUF - bo;
       if (has_group(k)) mbar_wait(&bars[s], mph);
       if (k <= z1) {
         if (k - 1 >= z0) { phase_D(IC<0>(), g0, bn, eoff, emask, esign); phase_D(IC<2>(), g0, bn, eoff, emask, esign); }
-        phase_B(IC<0>(), IC<0>(), p0, g0, k, s, bo, bn);
-        phase_B(IC<0>(), IC<2>(), p1, g0, k, s, bo, bn);
+        const V f0 = phase_B(IC<0>(), IC<0>(), p0, g0, k, s, bo, bn);
+        const V f1 = phase_B(IC<0>(), IC<2>(), p1, g0, k, s, bo, bn);
+        // a9: phi'(k-1) of the two pairs
+        const bool in0 = (unsigned)(k - 1 - pjlo) < (unsigned)pnjs0, in1 = (unsigned)(k - 1 - pjlo) < (unsigned)pnjs1;
+        stg_pair_if(in0, pph, f0);
+        stg_pair_if(in1, pph + 2 * L.px, f1);
+        if (img0 || img1 || SLAB) {
+          V o[NF_MAX];
+          if (in0) { o[F_PHI] = f0; store_rare<T, FM_PHI, SLAB>(P, o, k - 1, gx_, gy_, img0); }
+          if (in1) { o[F_PHI] = f1; store_rare<T, FM_PHI, SLAB>(P, o, k - 1, gx_, gy_ + 2, img1); }
+        }
       }
-      iter_end(k);
+      pph += L.plane;
+      iter_end(IC<0>(), k);
     }
   }
 }
