@@ -113,8 +113,7 @@ struct TileCfg {
   static constexpr int B_GQ = B_ZZ + (TWO ? 3 * ZLE : 0);        // [2]  phi + q_y, phi - q_y
   static constexpr int B_FQ = B_GQ + (TWO ? 2 * GQE : 0);        // [2]  (phi + q_x).y, (phi - q_x).x per pair
   static constexpr int B_KF = B_FQ + (TWO ? 2 * FQE : 0);        // [3]  F = sigma kappa grad(phi), phase -> flow
-  static constexpr int B_GR = B_KF + (TWO ? 3 * TLE : 0);        // [3]  grad(phi), private to the owning phase thread
-  static constexpr int B_PH = B_GR + (TWO ? 3 * TLE : 0);        // [1]  own phi, private to the owning phase thread
+  static constexpr int B_PH = B_KF + (TWO ? 3 * TLE : 0);        // [1]  own phi, private to the owning phase thread
   static constexpr int BUF = (B_PH + (TWO ? TLE : 0) + 3) / 4 * 4;   // elements per half
   static_assert(ZCE % 2 == 0 && ZLE % 2 == 0 && GQE % 2 == 0 && FQE % 2 == 0, "pair alignment");
   // y-push field: TY sending rows, and one more row that holds the x-pass terms of a halo column for the
@@ -127,7 +126,10 @@ struct TileCfg {
   static constexpr size_t OFF_BUF = OFF_PHI + (TWO ? S * PHI_STAGE : 0);    // [2][BUF]
   // y-push fields: a+ of region rows 0..TY-1 and a- of region rows 2..TY+1 (written and read inside one
   // iteration, between the x-pass barrier and the CTA barrier)
-  static constexpr size_t OFF_AP = OFF_BUF + (size_t)2 * BUF * sizeof(T);   // [9]
+  // grad(phi) of the tile nodes, written by the phase thread that owns the pair and read two iterations
+  // later by whoever forms F: a ring of three slots (slot = TMA ring slot of the writing iteration)
+  static constexpr size_t OFF_GR = OFF_BUF + (size_t)2 * BUF * sizeof(T);   // [3][3][TLE]
+  static constexpr size_t OFF_AP = OFF_GR + (TWO ? (size_t)9 * TLE * sizeof(T) : 0);   // [9]
   static constexpr size_t OFF_AM = OFF_AP + (size_t)NYP * YPF * sizeof(T);  // [9]
   static constexpr size_t OFF_BAR = OFF_AM + (size_t)NYP * YPF * sizeof(T);
   static constexpr size_t SMEM_BYTES = OFF_BAR + 64;
@@ -318,6 +320,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   auto mom_at = [&](int slot) { return reinterpret_cast<T *>(smem + C::OFF_MOM + slot * C::MOM_STAGE); };
   auto phi_at = [&](int slot) { return reinterpret_cast<T *>(smem + C::OFF_PHI + slot * C::PHI_STAGE); };
   T *s_buf = reinterpret_cast<T *>(smem + C::OFF_BUF);     // [2][BUF]
+  T *s_gr = reinterpret_cast<T *>(smem + C::OFF_GR);       // [3][3][TLE]
   T *s_ap = reinterpret_cast<T *>(smem + C::OFF_AP);       // [9][YPF]
   T *s_am = reinterpret_cast<T *>(smem + C::OFF_AM);
 
@@ -334,8 +337,8 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
                               : (colw ? (lane < RY ? lane : (lane < 2 * RY ? lane - RY : 0)) : 4 * (wid - C::W_PH0) + 1 + hi));
   const int cside = lane >= RY;                           // halo-column warp: 0 left, 1 right
   const int c0 = colw ? (cside ? HL + TX : HL - 2) : HL + 2 * lx;
-  const int oM = r * RX + c0;                             // offset of the pair in a staged region plane
-  const int oT = (r - 1) * TX + 2 * lx;                   // ... in an array over the tile
+  int oM = r * RX + c0;                                   // offset of the pair in a staged region plane
+  int oT = (r - 1) * TX + 2 * lx;                         // ... in an array over the tile
   // Tile origin.  When nx (ny) is not a multiple of the tile, the last tile of the row (column) is
   // shifted back to end at the domain edge; it recomputes the overlap but stores only its own nodes.
   const int xs = (blockIdx.x % M.ntx) * TX, ys = (blockIdx.x / M.ntx) * TY;
@@ -459,8 +462,8 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     }
     if (ROLE == 0) {
       const V qz = pfma(bq, st.nB[2], a4 * lds_pair(mo + F_UZ * MF));
-      // grad(phi) of plane k+1 for the kick two iterations on: private two-slot ring (slot = plane parity)
-      T *gr_ = s_buf + bn + C::B_GR + g.oT;
+      // grad(phi) of plane k+1 for the kick two iterations on -> ring slot s
+      T *gr_ = s_gr + s * 3 * TLE + g.oT;
       sts_pair(gr_, gx); sts_pair(gr_ + TLE, gy); sts_pair(gr_ + 2 * TLE, gz);
       // phi'(k-1) = phi/4 + (in-plane arrivals of plane k-1 + up(k-2) + down(k)) / 8
       const T *fr = s_buf + bn + C::B_FQ + g.oF;
@@ -475,12 +478,13 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     return phinew;
   };
 
-  // D: kappa(k-1) = -(S_y ax + D_y bx + S_y cx) from the x-combined z-combinations of n written in iteration
-  // k-1, plus the share of the halo column for the lanes at the tile edge (every other lane reads zeros
+  // D (run for half of the tile pairs by the phase warp that owns them, for the other half by the halo-row
+  // warp, which has time to spare): kappa(k-1) = -(S_y ax + D_y bx + S_y cx) from the x-combined
+  // z-combinations of n written in iteration k-1, plus the share of the halo column for the lanes at the tile edge (every other lane reads zeros
   // through the same per-lane pointer: no divergence); F(k-1) = sigma kappa grad(phi)(k-1) -> flow warps.
-  auto phase_D = [&](auto drc, const PairGeom &g0, int bn, int eoff, V emask, T esign) {
+  auto phase_D = [&](auto drc, int oZ0, int oT0, int s, int bn, int eoff, V emask, T esign) {
     constexpr int DR = decltype(drc)::value;
-    const PairGeom g = {0, 0, 0, 0, g0.oZ + DR * ZW, 0, 0, g0.oT + DR * TX};
+    const PairGeom g = {0, 0, 0, 0, oZ0 + DR * ZW, 0, 0, oT0 + DR * TX};
     const T *zr = s_buf + bn + C::B_ZC + g.oZ;
     V kap = pfma(lds_pair(zr), w0, (lds_pair(zr - ZW) + lds_pair(zr + ZW)) * w1);                       // S_y D_x a
     kap = pfma(lds_pair(zr + ZCE + ZW) - lds_pair(zr + ZCE - ZW), T(0.5), kap);                         // D_y S_x b
@@ -492,7 +496,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     const T corr = esign * ea + T(1.0 / 12.0) * eb + w1 * ec;            // -+ a/2 (D_x), w1 b and w1 c (S_x)
     kap = pfma(V(corr), emask, kap);
     const V sc = kap * (-P.sigma);                                       // F = sigma kappa G, kappa = -kap
-    const T *gr_ = s_buf + bn + C::B_GR + g.oT;
+    const T *gr_ = s_gr + (s == S - 1 ? 0 : s + 1) * 3 * TLE + g.oT;      // G(k-1): written two iterations ago
     T *kf = s_buf + bn + C::B_KF + g.oT;
     sts_pair(kf, lds_pair(gr_) * sc);
     sts_pair(kf + TLE, lds_pair(gr_ + TLE) * sc);
@@ -516,14 +520,20 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   // (same warp); the lanes at the tile edge take the halo column's term, which the halo-column warp left in
   // the extra row of the same fields one iteration earlier.
   const bool st_ap = r <= TY - 1, st_am = r >= 2;        // rows 0..TY-1 send an a+, rows 2..TY+1 an a-
+  // y-push fields: a+ is stored at row index r, a- at r-2; a tile row r reads both at index r-1 (= oT)
+  int oAP = r * TX + 2 * lx;
+  // x-exchange word of this lane: word `lane` of a row of the y-push fields 0..7 that this warp is about
+  // to overwrite (a+ field: the warp's first sending row; a- field: its last)
+  int oXP = (flow ? 2 * wid + 1 : 0) * TX + lane, oXM = (flow ? 2 * wid : TY - 1) * TX + lane;
+  // the word it reads: its x neighbour's, or (lanes at the tile edge) the halo-column term of row r in the
+  // extra row of the same field (+ RY for planes of odd parity)
+  int oPL = lx == 0 ? TY * TX + r : oXP - 1, oPR = lx == LX - 1 ? TY * TX + r : oXM + 1;
+  const int hpar = (lx == 0 ? 1 : 0) | (lx == LX - 1 ? 2 : 0);
   auto xpass = [&](int k, int s, V (&A0)[9]) {
-    // y-push fields: a+ is stored at row index r, a- at r-2; a tile row r reads both at index r-1 (= oT)
-    const int oAP = r * TX + 2 * lx, oAM = oAP - 2 * TX;
-    // x-exchange word of this lane: word `lane` of a row of the y-push fields 0..7 that this warp is about
-    // to overwrite (a+ field: the warp's first sending row; a- field: its last)
-    T *const xp = s_ap + (flow ? 2 * wid + 1 : 0) * TX + lane, *const xm = s_am + (flow ? 2 * wid : TY - 1) * TX + lane;
-    const int hrow = TY * TX + (k & 1) * RY + r;         // the halo-column terms of plane k, row r
-    const T *pl = lx == 0 ? s_ap + hrow : xp - 1, *pr = lx == LX - 1 ? s_am + hrow : xm + 1;
+    const int oAM = oAP - 2 * TX;
+    T *const xp = s_ap + oXP, *const xm = s_am + oXM;
+    const int hoff = (k & 1) * RY;
+    const T *pl = s_ap + oPL + ((hpar & 1) ? hoff : 0), *pr = s_am + oPR + ((hpar & 2) ? hoff : 0);
     V Xg[8][3];   // [group][p]
     {
       V m[10], K[NK];
@@ -576,7 +586,14 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     const int jlo = max(z0, P.jet_lo ? 1 : 0);
     const int njs = (gx_ >= xs && gy_ >= ys) ? min(z1, P.out_hi ? L.nz - 1 : L.nz) - jlo : 0;
     T *pst = P.out.f[0] + o00 + (long long)(kst - 2) * L.plane;   // field 0 of the pair, plane k-2
+    // halo-row warp: D for the second pair of every phase thread (tile rows 3 + hi and 7 + hi)
+    const int dZ = (3 + hi) * ZW + 2 + 2 * lx, dT = (2 + hi) * TX + 2 * lx;
+    const int deoff = (lx == 0 ? C::B_ZL : (lx == LX - 1 ? C::B_ZL + RY : C::B_ZZ)) + 2 + 3 + hi;
+    const V demask(lx == 0 ? T(1) : T(0), lx == LX - 1 ? T(1) : T(0));
+    const T design = lx == 0 ? T(-0.5) : T(0.5);
     for (int i = 0; i < NI; ++i) {
+      // (keep the loop-invariant offsets in registers: recomputing them from the thread index costs more)
+      asm volatile("" : "+r"(oM), "+r"(oT), "+r"(oAP), "+r"(oXP), "+r"(oXM), "+r"(oPL), "+r"(oPR));
       const int k = kst + i;
       const int bo = (k & 1) * BUF;          // exchange-block half of this plane's parity
       if (has_group(k)) mbar_wait(&bars[s], mph);
@@ -584,6 +601,10 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
       V A0[9];                               // own y-push term a0 per (c,p)
       if (src) xpass(k, s, A0);
       xpass_barrier();
+      if (TWO && halow && k <= z1 && k - 1 >= z0) {
+        phase_D(IC<0>(), dZ, dT, s, BUF - bo, deoff, demask, design);
+        phase_D(IC<4>(), dZ, dT, s, BUF - bo, deoff, demask, design);
+      }
       V o[NF_MAX];
       if (TWO && flow && (unsigned)(k - 2 - jlo) < (unsigned)njs) {
         // a6: u'(k-2) = u_b + F / rho' with the F(k-2) the phase warps wrote in iteration k-1; a9: store it
@@ -716,7 +737,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
       const int bo = (k & 1) * BUF, bn = BUF - bo;
       if (has_group(k)) mbar_wait(&bars[s], mph);
       if (k <= z1) {
-        if (k - 1 >= z0) { phase_D(IC<0>(), g0, bn, eoff, emask, esign); phase_D(IC<2>(), g0, bn, eoff, emask, esign); }
+        if (k - 1 >= z0) phase_D(IC<0>(), g0.oZ, g0.oT, s, bn, eoff, emask, esign);   // (rows r + 2: the halo-row warp)
         const V f0 = phase_B(IC<0>(), IC<0>(), p0, g0, k, s, bo, bn);
         const V f1 = phase_B(IC<0>(), IC<2>(), p1, g0, k, s, bo, bn);
         // a9: phi'(k-1) of the two pairs
