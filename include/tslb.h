@@ -132,6 +132,22 @@ int tslb_get_moments(tslb_ctx *c, void *rho, void *ux, void *uy, void *uz, void 
  * stream.  Not available on a z-slab (TSLB_EINVAL).                                              */
 int tslb_get_physical_velocity(tslb_ctx *c, void *ux, void *uy, void *uz, int pointers_on_device);
 
+/* The same velocity for callers that must not allocate (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): this entry point calls no cudaMalloc, cudaFree or allocating
+ * library routine.  ux, uy, uz are DEVICE pointers (dense, nx*ny*nz elements of the context's precision;
+ * any may be NULL); the call is asynchronous on the context's stream and does NOT synchronise it.  The
+ * scratch it needs (the three normal arrays n = grad(phi)/(|grad(phi)|+eps), eqs. 20-21,
+ * of the padded grid) is one file-scope device array of tslb_noalloc_scratch_bytes() = 12 MiB that every
+ * GPU holds from the moment it loads the library until the process exits; its device address is resolved
+ * once per device (cudaGetSymbolAddress) when a context is created there.  Grids that need more --
+ * 3 * (nx+16)*(ny+4)*nz elements, each array rounded up to 256 bytes -- are rejected with TSLB_EINVAL and
+ * a message (about 1.0 M padded nodes in fp32, 0.5 M in fp64: e.g. 64x64x128 fp32, 64^3 fp64).  All
+ * contexts on a device SHARE the array and it keeps the last call's contents (every entry a call reads
+ * it has written first, so nothing is cleared): two calls that overlap on the GPU -- different streams,
+ * or different contexts on one device -- race; serialise them.  TSLB_EINVAL on a z-slab.             */
+int tslb_get_physical_velocity_noalloc(tslb_ctx *c, void *ux, void *uy, void *uz);
+size_t tslb_noalloc_scratch_bytes(void);
+
 /* ---- z-slabs: one domain split along z over several contexts / GPUs (the paper's
  * stated next step).  Every node update reads only time-t values within one
  * plane (moments) / two planes (phi) of itself, so a slab needs, per step and per shared face, the

@@ -365,6 +365,58 @@ int get_typed(tslb_ctx *c, void *const dst[NF_MAX], int on_device) {
   return TSLB_OK;
 }
 
+
+// ---- tslb_get_physical_velocity_noalloc: scratch that nobody allocates.
+// The three normal arrays n = grad(phi)/(|grad(phi)|+eps) of phase_normals_kernel live in ONE file-scope
+// device array of a fixed, modest size: every GPU that loads the library holds it until the process
+// exits.  In host code the array's NAME is only a stand-in, not a device address: a kernel given it
+// would fault (or, where the GPU can reach host memory, silently use the wrong memory).  The device
+// address comes from cudaGetSymbolAddress, asked once per device with that device current.
+constexpr size_t NOALLOC_SCRATCH_BYTES = (size_t)12 << 20;   // 12 MiB: 3 arrays of <= 4 MiB each
+static __device__ __align__(256) unsigned char g_noalloc_scratch[NOALLOC_SCRATCH_BYTES];
+void *g_noalloc_ptr[TSLB_MAX_DEVICES] = {};                   // device address of the array, per device
+
+// device must be the current device
+cudaError_t noalloc_scratch_address(int device, void **out) {
+  if (device < 0 || device >= TSLB_MAX_DEVICES) return cudaErrorInvalidDevice;
+  if (!g_noalloc_ptr[device]) {
+    void *ptr = nullptr;
+    cudaError_t e = cudaGetSymbolAddress((void **)&ptr, g_noalloc_scratch);
+    if (e != cudaSuccess) return e;
+    g_noalloc_ptr[device] = ptr;
+  }
+  *out = g_noalloc_ptr[device];
+  return cudaSuccess;
+}
+
+template <typename T>
+int physvel_noalloc_typed(tslb_ctx *c, void *const dst[3], void *scratch) {
+  const Layout &L = c->v.L;
+  const bool guo = c->p.forcing == TSLB_FORCING_GUO;
+  const bool use_force = c->p.two_component && (guo || c->t >= 1);
+  // GUO: F of the current phi; KICK: F of the previous step's phi, still in the other buffer
+  const int src = guo ? c->cur : c->cur ^ 1;
+  StepParams<T> P = make_step_params<T>(c, src, src);
+  for (int side = 0; side < 2; ++side)
+    for (int k = 0; k < NF_MAX; ++k) P.nb[side].f[k] = nullptr;
+  const size_t fb = round_up((size_t)L.field * sizeof(T), 256);
+  for (int k = 0; k < 3; ++k) P.nrm[k] = (T *)((char *)scratch + k * fb);
+  dim3 b(32, 8), g((L.nx + 31) / 32, (L.ny + 7) / 8, L.nz);
+  if (use_force) {
+    // every entry of n that physical_velocity_kernel reads (the 27 neighbours of every node, by index
+    // arithmetic: wrapped in x, y, wrapped or clamped in z) is written here first: nothing in the scratch
+    // needs to start at zero, and the last call's contents are simply overwritten
+    phase_normals_kernel<T><<<g, b, 0, c->stream>>>(P);
+    CK(cudaGetLastError());
+  }
+  FieldSet<T> vel;
+  for (int k = 0; k < NF_MAX; ++k) vel.f[k] = (T *)c->fields[c->cur][k];
+  physical_velocity_kernel<T><<<g, b, 0, c->stream>>>(P, vel, guo ? T(0.5) : T(-0.5), use_force ? 1 : 0, (T *)dst[0],
+                                                      (T *)dst[1], (T *)dst[2]);
+  CK(cudaGetLastError());
+  return TSLB_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -393,6 +445,12 @@ int tslb_create(const tslb_params *p, tslb_ctx **out) {
   if (prop.major != 10) {
     g_create_error = "this library is built for sm_100a (B200) only";
     return TSLB_ECUDA;
+  }
+  {
+    // set-up of the allocation-free entry point: the device address of its scratch array, once per device
+    // (a failure here is reported by tslb_get_physical_velocity_noalloc, which asks again)
+    void *scratch = nullptr;
+    if (noalloc_scratch_address(p->device, &scratch) != cudaSuccess) cudaGetLastError();
   }
   tslb_ctx *c = new (std::nothrow) tslb_ctx();
   if (!c) { g_create_error = "out of host memory"; return TSLB_ENOMEM; }
@@ -500,6 +558,26 @@ int tslb_get_physical_velocity(tslb_ctx *c, void *ux, void *uy, void *uz, int po
   return c->p.precision == TSLB_F32 ? physvel_typed<float>(c, dst, pointers_on_device)
                                     : physvel_typed<double>(c, dst, pointers_on_device);
 }
+
+int tslb_get_physical_velocity_noalloc(tslb_ctx *c, void *ux, void *uy, void *uz) {
+  if (!c) return TSLB_EINVAL;
+  if (!c->inited) return c->fail(TSLB_ESTATE, "tslb_get_physical_velocity_noalloc before tslb_init_fields");
+  if (c->v.slab) return c->fail(TSLB_EINVAL, "tslb_get_physical_velocity_noalloc is not available on a z-slab");
+  const size_t need = 3 * round_up((size_t)c->v.L.field * c->v.esize, 256);
+  if (need > NOALLOC_SCRATCH_BYTES)
+    return c->fail(TSLB_EINVAL,
+                   "tslb_get_physical_velocity_noalloc: the grid needs %zu bytes of scratch, the built-in array holds %zu "
+                   "(use tslb_get_physical_velocity)", need, (size_t)NOALLOC_SCRATCH_BYTES);
+  CK(cudaSetDevice(c->p.device));
+  void *scratch = nullptr;
+  cudaError_t e = noalloc_scratch_address(c->p.device, &scratch);
+  if (e != cudaSuccess) return c->cuda_fail(e, "cudaGetSymbolAddress(scratch)");
+  void *dst[3] = {ux, uy, uz};
+  return c->p.precision == TSLB_F32 ? physvel_noalloc_typed<float>(c, dst, scratch)
+                                    : physvel_noalloc_typed<double>(c, dst, scratch);
+}
+
+size_t tslb_noalloc_scratch_bytes(void) { return NOALLOC_SCRATCH_BYTES; }
 
 void *tslb_workspace_ptr(const tslb_ctx *c) { return c ? c->ws : nullptr; }
 

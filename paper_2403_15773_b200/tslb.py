@@ -19,7 +19,8 @@ KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED = 0, 1, 2
 FORCING_KICK, FORCING_GUO = 0, 1
 
 EXPORTS = ["tslb_workspace_bytes", "tslb_create", "tslb_init_fields", "tslb_step",
-           "tslb_get_moments", "tslb_get_physical_velocity", "tslb_step_count", "tslb_kernel_name", "tslb_launch_count",
+           "tslb_get_moments", "tslb_get_physical_velocity", "tslb_get_physical_velocity_noalloc",
+           "tslb_noalloc_scratch_bytes", "tslb_step_count", "tslb_kernel_name", "tslb_launch_count",
            "tslb_debug_xi", "tslb_destroy", "tslb_last_error", "tslb_workspace_ptr",
            "tslb_attach_neighbor", "tslb_ipc_get_handle", "tslb_attach_neighbor_ipc", "tslb_halo_push",
            "tslb_stats_begin", "tslb_stats_get", "tslb_stats_end"]
@@ -69,6 +70,9 @@ def lib():
         L.tslb_step.argtypes = [vp, ctypes.c_int]
         L.tslb_get_moments.argtypes = [vp, vp, vp, vp, vp, ctypes.POINTER(vp), vp, ctypes.c_int]
         L.tslb_get_physical_velocity.argtypes = [vp, vp, vp, vp, ctypes.c_int]
+        L.tslb_get_physical_velocity_noalloc.argtypes = [vp, vp, vp, vp]
+        L.tslb_noalloc_scratch_bytes.argtypes = []
+        L.tslb_noalloc_scratch_bytes.restype = ctypes.c_size_t
         L.tslb_step_count.argtypes = [vp]
         L.tslb_step_count.restype = ctypes.c_longlong
         L.tslb_kernel_name.argtypes = [vp]
@@ -236,6 +240,13 @@ class Tslb:
             ptrs = [u[a].ctypes.data for a in range(3)]
         self._check(lib().tslb_get_physical_velocity(self._h, ptrs[0], ptrs[1], ptrs[2], int(device)))
         return u
+
+    def get_physical_velocity_noalloc(self, out):
+        """The same into `out`, a (3, nz, ny, nx) torch CUDA tensor of the context's dtype, through the entry
+        point that allocates nothing (built-in scratch array; small grids only).  Asynchronous."""
+        assert tuple(out.shape) == (3,) + self.shape and out.dtype == self.torch_dtype and out.is_cuda and out.is_contiguous()
+        self._check(lib().tslb_get_physical_velocity_noalloc(self._h, out[0].data_ptr(), out[1].data_ptr(), out[2].data_ptr()))
+        return out
 
     # -- z-slabs (include/tslb.h "z-slabs")
     @property
