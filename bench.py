@@ -7,7 +7,10 @@ flow + phase-field step and achieved HBM GB/s against the B200 peak).
 A "step" is one pass of the whole hot path over the full lattice.
 N = 1 runs BASELINE.json configs[4] ("c5": 512x512x1536 fp32 jet, 402 653 184 nodes), the
 configuration the metric is quoted on.  N > 1 (torchrun) runs N independent replicas of the same
-workload, one per GPU ("replicas only"): the path has no exchange step yet.
+workload, one per GPU ("replicas only", the default, weak scaling), or with --decomp slabs ONE domain
+split into z-slabs whose step kernels push their halo planes into the neighbours' ghost planes
+(strong scaling).  The timed region (exactly K steps between CUDA events on the library's
+stream) is repeated --reps times; `value` is the median, `reps` lists every repetition.
 Prints ONE JSON line (rank 0).
 """
 import argparse
@@ -52,6 +55,8 @@ def parse():
                     help="how the surface-tension force enters (include/tslb.h): the kick of reading A9 (default, all "
                          "kernels) or the Guo-type forcing of reading A18 (generic kernel only; its cost is a bench line "
                          "of its own, not the headline)")
+    ap.add_argument("--reps", type=int, default=3, help="repetitions of the timed region of K steps (value = median)")
+    ap.add_argument("--sample", default="slab", help="(--impl cpu-sample) oracle sample: slab | c3 | c4slab")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     return ap.parse_args()
@@ -153,20 +158,28 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------ CPU oracle legs
-def oracle_sample(cfg_name, steps):
-    """Time the oracle, as it stands, on a bounded slab of the same workload.
-    -> (GLUPS, threads, description)"""
+def oracle_sample(cfg_name, steps, sample="slab"):
+    """Time the oracle, as it stands, on a bounded sample of the workload.
+    sample: "slab" = the first 16 planes of the bench configuration (64^3 sub-box for c3); "c3" = BASELINE
+    configs[2] in full (128^3 droplets + noise); "c4slab" = the first 128 planes of configs[3] (256x256x512 jet).
+    -> (GLUPS, threads, description, seconds per step)"""
     from oracle import ref
     from paper_2403_15773_b200 import inputs
     nx, ny, nz, D, _ = CONFIGS[cfg_name]
-    if cfg_name == "c3":
-        n = 64
-        d = inputs.droplets_noise(n, seed=12345, ndrop=5)
+    if sample == "c3" or (sample == "slab" and cfg_name == "c3"):
+        n = 128 if sample == "c3" else 64
+        d = inputs.droplets_noise(n, seed=12345, ndrop=40 if n == 128 else 5)
         o = ref.Oracle(n, n, n, 1.95, two_component=True, sigma=0.005, interface_width=4.0)
-        desc = "64^3 sub-box of the C3 recipe (5 droplets + noise), %d steps" % steps
+        desc = ("C3 in full: 128^3 periodic, 40 droplets + noise, %d steps" % steps) if n == 128 else \
+               ("64^3 sub-box of the C3 recipe (5 droplets + noise), %d steps" % steps)
         nodes = n ** 3
     else:
-        sz = 16
+        if sample == "c4slab":
+            cfg_name = "c4"
+            nx, ny, nz, D, _ = CONFIGS["c4"]
+            sz = 128
+        else:
+            sz = 16
         prm = inputs.jet_params(nx, ny, sz, D, We=200.0 if cfg_name == "c4" else 2000.0)
         d = inputs.jet_developed(nx, ny, sz, D, ndrop=4)
         o = ref.Oracle(nx, ny, sz, prm["omega"], two_component=True, sigma=prm["sigma"], interface_width=4.0,
@@ -181,6 +194,24 @@ def oracle_sample(cfg_name, steps):
     dt = time.perf_counter() - t0
     o.close()
     return nodes * steps / dt / 1e9, ref.num_threads(), desc, dt / steps
+
+
+def cpu_sample_subprocess(cfg_name, steps, sample, threads):
+    """The same in a child process with OMP_NUM_THREADS fixed (OpenMP reads it once per process).
+    threads = 0: all cores.  -> dict or None"""
+    env = dict(os.environ)
+    if threads:
+        env["OMP_NUM_THREADS"] = str(threads)
+    else:
+        env.pop("OMP_NUM_THREADS", None)
+    for k in ("RANK", "WORLD_SIZE", "LOCAL_RANK"):
+        env.pop(k, None)
+    try:
+        r = subprocess.run([sys.executable, os.path.abspath(__file__), "--impl", "cpu-sample", "--config", cfg_name,
+                            "--steps", str(steps), "--sample", sample], env=env, capture_output=True, text=True, timeout=600)
+        return json.loads(r.stdout.strip().splitlines()[-1])
+    except Exception as ex:      # the baseline is a report, not a gate
+        return {"error": repr(ex)[:200], "sample": sample, "threads": threads}
 
 
 def cpu_model():
@@ -198,11 +229,13 @@ def run_reference(args):
     if rank != 0:
         return
     nx, ny, nz, D, desc = CONFIGS[args.config]
-    # each "step" of this arm is one oracle time step on the bounded slab
+    # each "step" of this arm is one oracle time step on the bounded slab; at most 4 are run (a step takes
+    # seconds), after one untimed step that pages the state in -- the line reports what ran
     steps = max(1, min(args.steps, 4))
     glups, threads, sample, sps = oracle_sample(args.config, steps)
     out = {"impl": "reference", "metric": "GLUPS (fused flow+phase-field step)", "value": glups, "unit": "GLUPS",
-           "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": sps * 1e3,
+           "n_gpus": args.gpus, "steps": steps, "warmup": 1, "requested": {"steps": args.steps, "warmup": args.warmup},
+           "ms_per_step": sps * 1e3,
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
            "config": {"workload": desc, "grid": [nx, ny, nz]},
            "cpu_baseline": {"value": glups, "unit": "GLUPS", "cores": threads, "kind": "oracle", "sample": sample,
@@ -306,6 +339,10 @@ def main():
     if args.impl == "reference":
         run_reference(args)
         return
+    if args.impl == "cpu-sample":            # child of the cpu_baseline leg (fixed OMP_NUM_THREADS)
+        g, threads, sample, sps = oracle_sample(args.config, max(1, args.steps), args.sample)
+        print(json.dumps({"value": g, "unit": "GLUPS", "cores": threads, "sample": sample, "s_per_step": sps}))
+        return
     if args.decomp == "slabs":
         run_slabs(args)
         return
@@ -357,21 +394,24 @@ def main():
     sampler.start()
     time.sleep(0.25)
     l0 = sim.launch_count
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     t0 = time.time()
-    e0.record()
-    sim.step(args.steps)
-    e1.record()
-    barrier()
+    rep_ms = []
+    for _ in range(max(1, args.reps)):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        sim.step(args.steps)
+        e1.record()
+        barrier()
+        rep_ms.append(tdist.max_over_ranks(e0.elapsed_time(e1), dev))
     t1 = time.time()
     clocks = sampler.stop(t0, t1)
-    ms = e0.elapsed_time(e1)
-    launches = sim.launch_count - l0
+    ms = float(np.median(rep_ms))            # K steps, median over the repetitions (max over ranks each)
+    launches = (sim.launch_count - l0) // max(1, args.reps)
     m = sim.get_moments(device=True, want=("rho", "phi"))
     finite = bool(torch.isfinite(m["rho"]).all().item() and torch.isfinite(m["phi"]).all().item())
     del m
-    ms_max = tdist.max_over_ranks(ms, dev)
-    glups = tdist.job_throughput(nodes * args.steps, ms * 1e-3, dev) / 1e9
+    ms_max = ms
+    glups = world * nodes * args.steps / (ms * 1e-3) / 1e9      # whole job: all ranks' nodes / slowest rank's time
 
     # ---- end to end through the C-ABI with HOST buffers: H2D of the inputs, K steps, D2H of the state
     e2e = None
@@ -435,16 +475,22 @@ def main():
     if not args.no_cpu:
         g, threads, sample, _ = oracle_sample(args.config, 6)
         cpu = {"value": g, "unit": "GLUPS", "cores": threads, "kind": "oracle", "sample": sample,
-               "cpu_model": cpu_model()}
+               "cpu_model": cpu_model(),
+               # the oracle on C3 and on the C4 shape, one thread and all cores (bounded:
+               # each child runs a few seconds to half a minute)
+               "more": [cpu_sample_subprocess("c3", 10, "c3", 0), cpu_sample_subprocess("c3", 2, "c3", 1),
+                        cpu_sample_subprocess("c4", 2, "c4slab", 0), cpu_sample_subprocess("c4", 1, "slab", 1)]}
 
     out = {"metric": "GLUPS (fused flow+phase-field step)", "value": glups, "unit": "GLUPS", "n_gpus": world,
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
-           "scaling": "weak", "vs_baseline": (glups / 2.0 if args.config == "t1" and world == 1 else None), "dtype": args.precision, "data": "synthetic",
+           "scaling": "weak", "vs_baseline": None, "dtype": args.precision, "data": "synthetic",
            "config": {"workload": desc, "grid": [nx, ny, nz], "state_bytes_per_gpu": 2 * 11 * nodes * (4 if prec == tslb.F32 else 8),
-                      "l2": "state (%.1f GB) far exceeds the 126 MB L2; no flush needed" % (2 * 11 * nodes * 4 / 1e9),
+                      "l2": "state (%.1f GB) far exceeds the 126 MB L2; no flush needed" % (2 * 11 * nodes * (4 if prec == tslb.F32 else 8) / 1e9),
                       "parallelism": "replicas x%d" % world if world > 1 else "single GPU",
                       "initial_state": "seeded synthetic developed jet (device-generated)", "finite": finite,
                       "forcing": args.forcing},
+           "reps": {"n": len(rep_ms), "ms_per_step": [x / args.steps for x in rep_ms], "median": ms / args.steps,
+                    "min": min(rep_ms) / args.steps},
            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
            "paper_context": "paper: ~1.5 GLUPS RTX 3090, ~2 GLUPS A100 on 400x400x800 (PAPER.md:283); other hardware, not the target"}
     print(json.dumps(out))

@@ -331,7 +331,9 @@ def test_p12_gradient_stencil_fourier_symbol_and_curvature():
 # ---------------------------------------------------------------- jet boundaries (A10/A11: parity unpinned)
 def test_jet_boundary_planes_sanity():
     """Inflow/outflow (eqs. 9-10 as read in A10/A11): imposed values are what is
-    stored, inlet mass flux = sum_nozzle rho U (1 + p xi), fields stay bounded."""
+    stored, one-step memory of the neighbour plane, fields stay bounded.  (The rebuilt populations and the
+    mass / momentum fluxes through the two planes: test_jet_boundary_populations_are_eq9,
+    test_jet_mass_balance_from_boundary_populations.)"""
     nx, ny, nz, D, U, pert, seed = 24, 24, 40, 8.0, 0.05, 0.05, 2024
     prm = inputs.jet_params(nx, ny, nz, D, U=U, Re=500.0, We=200.0, perturbation=pert, seed=seed)
     d = inputs.jet_quiescent(nx, ny, nz)
@@ -362,3 +364,110 @@ def test_jet_boundary_planes_sanity():
     assert 0.97 < m["rho"].min() and m["rho"].max() < 1.03
     assert m["phi"][1:6].sum() > 100           # fluid A has entered
     assert np.isfinite(m["pineq"]).all()
+
+
+def _jet_oracle(nx, ny, nz, D, forcing=None, steps=0, seed=2024, pert=0.05, U=0.05):
+    prm = inputs.jet_params(nx, ny, nz, D, U=U, Re=300.0, We=20.0, perturbation=pert, seed=seed)
+    d = inputs.jet_developed(nx, ny, nz, D, U=U, ndrop=3)
+    rng = np.random.default_rng(11)
+    for k in ("ux", "uy"):      # transverse motion, so that Pi^neq and u differ from plane to plane
+        d[k] = 0.01 * rng.standard_normal(d[k].shape)
+    kw = {} if forcing is None else dict(forcing=forcing)
+    o = ref.Oracle(nx, ny, nz, prm["omega"], two_component=True, sigma=prm["sigma"], interface_width=4.0,
+                   bc_zlo=ref.BC_JET_INFLOW, bc_zhi=ref.BC_OUTFLOW, jet_diameter=D, jet_velocity=U,
+                   jet_perturbation=pert, seed=seed, **kw)
+    o.init_fields(d["rho"], d["ux"], d["uy"], d["uz"], d["phi"])
+    if steps:
+        o.step(steps)
+    return o, prm
+
+
+def test_jet_boundary_populations_are_eq9():
+    """PAPER.md:125-137 eqs. 9-10: f_i(x_B) = f_i^eq(rho_B, u_B) + (1 - omega) f_i^neq(Pi^neq(x_F), u_B) with the
+    IMPOSED rho_B, u_B of reading A10 and the neighbour plane's Pi^neq.  The populations the oracle holds
+    on the two boundary planes are compared with that formula rebuilt from the probes ref.feq / ref.fneq
+    (pinned by P2, P3).  A missing (1 - omega), a velocity taken from x_F, or a forgotten rebuild fails."""
+    nx, ny, nz, D = 20, 18, 16, 8.0
+    o, prm = _jet_oracle(nx, ny, nz, D, steps=3)
+    prev = o.get_moments()
+    o.step(1)
+    m = o.get_moments()
+    f = o.get_populations()
+    omc = 1.0 - prm["omega"]
+    assert abs(omc) > 0.3
+    worst = 0.0
+    for zb, zf in ((0, 1), (nz - 1, nz - 2)):
+        # the stored Pi^neq of the boundary plane is the OLD one of the fluid neighbour (A11), and it is not small
+        assert np.array_equal(m["pineq"][:, zb], prev["pineq"][:, zf])
+        assert np.abs(m["pineq"][:, zb]).max() > 1e-6
+        # the imposed velocity differs from the neighbour's
+        assert np.abs(m["uz"][zb] - m["uz"][zf]).max() > 1e-4
+        for y in range(ny):
+            for x in range(nx):
+                u = np.array([m["ux"][zb, y, x], m["uy"][zb, y, x], m["uz"][zb, y, x]])
+                want = ref.feq(m["rho"][zb, y, x], u) + omc * ref.fneq(m["pineq"][:, zb, y, x], u)
+                worst = max(worst, np.abs(f[:, zb, y, x] - want).max())
+    assert worst < 1e-15, worst
+    o.close()
+
+
+def test_jet_mass_balance_from_boundary_populations():
+    """Reading A10, its pin: the interior mass changes per step by exactly what the boundary-plane
+    populations carry in minus what the interior sends to the two planes, and the net inlet mass flux is
+    sum_nozzle rho_B U (1 + p xi)  (first moment of the rebuilt inlet populations = the imposed momentum)."""
+    nx, ny, nz, D, U, pert, seed = 20, 18, 16, 8.0, 0.05, 0.05, 2024
+    o, prm = _jet_oracle(nx, ny, nz, D, steps=2, U=U, pert=pert, seed=seed)
+    c, w = ref.lattice()
+    up, dn = c[:, 2] == 1, c[:, 2] == -1
+    x, y, _ = inputs.grid(nx, ny, 1)
+    disc = ((x[0] - (nx - 1) / 2) ** 2 + (y[0] - (ny - 1) / 2) ** 2) < (D / 2) ** 2
+    for t in (2, 3, 4):
+        m0 = o.get_moments()
+        f = o.get_populations()                       # post-collision populations of time t
+        assert abs(f[:, 1:-1].sum() - m0["rho"][1:-1].sum()) < 1e-10   # collision keeps the mass
+        o.step(1)
+        m1 = o.get_moments()
+        gain = f[up, 0].sum() + f[dn, nz - 1].sum()       # from the two boundary planes into planes 1 and nz-2
+        loss = f[dn, 1].sum() + f[up, nz - 2].sum()       # from planes 1 and nz-2 into the boundary planes
+        dm = m1["rho"][1:-1].sum() - m0["rho"][1:-1].sum()
+        assert abs(dm - (gain - loss)) < 1e-11 * max(gain, 1.0), (t, dm, gain - loss)
+        # net inlet flux = first z-moment of the inlet populations = imposed rho_B u_B
+        xi = np.array([[ref.xi(seed, i, j, nx, ny, t) for i in range(nx)] for j in range(ny)])
+        flux = (f[:, 0] * c[:, 2][:, None, None]).sum()
+        want = (m0["rho"][0] * np.where(disc, U * (1 + pert * xi), 0.0)).sum()
+        assert abs(flux - want) < 1e-13, (t, flux, want)
+        assert want > 0.5 * disc.sum() * U
+        # and no transverse momentum comes in
+        assert abs((f[:, 0] * c[:, 0][:, None, None]).sum()) < 1e-14
+    o.close()
+
+
+def test_guo_jet_momentum_balance_with_unforced_boundary_planes():
+    """Reading A18 with inflow/outflow: F = 0 on the two imposed planes.  (i) the first moment of the
+    boundary-plane populations is exactly the imposed rho_B u_B although grad(phi) is not zero there (nozzle
+    rim); (ii) the bare interior momentum obeys  sum m(t+1) = sum (m(t) + F(t)) + (what the boundary
+    populations carry in) - (what the interior sends out),  F = sigma kappa grad(phi) of the time-t phi."""
+    nx, ny, nz, D = 20, 18, 16, 8.0
+    o, prm = _jet_oracle(nx, ny, nz, D, forcing=ref.FORCING_GUO, steps=2)
+    c, w = ref.lattice()
+    up, dn = c[:, 2] == 1, c[:, 2] == -1
+    for t in (2, 3):
+        m0 = o.get_moments()
+        G, nn, kappa, F = o.phase_geometry()
+        assert np.abs(G[:, 0]).max() > 1e-3                # the nozzle rim: a force would be there
+        f = o.get_populations()
+        for zb in (0, nz - 1):
+            for a, key in enumerate(("ux", "uy", "uz")):
+                mom = (f[:, zb] * c[:, a][:, None, None]).sum(axis=0)
+                assert np.abs(mom - m0["rho"][zb] * m0[key][zb]).max() < 1e-16
+        o.step(1)
+        m1 = o.get_moments()
+        for a, key in enumerate(("ux", "uy", "uz")):
+            ca = c[:, a][:, None, None]
+            gain = (f[up, 0] * ca[up]).sum() + (f[dn, nz - 1] * ca[dn]).sum()
+            loss = (f[dn, 1] * ca[dn]).sum() + (f[up, nz - 2] * ca[up]).sum()
+            before = (m0["rho"][1:-1] * m0[key][1:-1]).sum() + F[a, 1:-1].sum()
+            after = (m1["rho"][1:-1] * m1[key][1:-1]).sum()
+            assert abs(after - (before + gain - loss)) < 1e-12, (t, key, after - (before + gain - loss))
+        assert np.abs(F[:, 1:-1]).max() > 1e-7
+    o.close()

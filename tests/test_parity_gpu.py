@@ -169,20 +169,49 @@ def oracle_sensitivity(tag, make_inputs, prm, steps):
     return _oracle_cache[key]
 
 
+def _golden_c2_conditioning():
+    """steps -> {field group: one-ulp divergence of two oracle runs} (tests/golden/c2_conditioning.txt)."""
+    p = os.path.join(os.path.dirname(__file__), "golden", "c2_conditioning.txt")
+    rows = {}
+    for line in open(p):
+        if line.startswith("#") or not line.strip():
+            continue
+        q = line.split()
+        rows[int(q[0])] = dict(rho=float(q[1]), u=float(q[2]), pineq=float(q[3]), phi=float(q[4]))
+    return rows
+
+
+C2_FACTOR = 3.0      # GPU-vs-oracle distance allowed, in units of the oracle's own one-ulp divergence (measured: 0.4 .. 1.3)
+
+
 @pytest.mark.parametrize("kernel", KERNELS)
 def test_c2_static_droplet_fp64(kernel):
     """BASELINE configs[1] (first 100 steps): two-component, fp64, 64^3, R=16, W=4, sigma=0.01.
-    1e-12 at 10 steps; at 100 steps 1e-12 or 10 x the oracle's own one-ulp sensitivity."""
+    north_star's 1e-12 holds while the step map is well conditioned (10 steps); from then on two runs of
+    the ORACLE itself whose inputs differ by one ulp drift apart (tests/golden/c2_conditioning.txt,
+    written by an oracle-only script), and the gate at 30, 50 and 100 steps is
+    max(1e-12, C2_FACTOR x that drift).  The achieved distances are printed (and recorded in DESIGN.md)."""
     prm = dict(nx=64, ny=64, nz=64, omega=1.0, two_component=True, sigma=0.01, interface_width=4.0)
-    mk = lambda: inputs.static_droplet(64, 16.0, 4.0)
-    check("c2", mk, prm, 10, tslb.F64, kernel)
-    sens = oracle_sensitivity("c2", mk, prm, 100)
-    print("oracle one-ulp sensitivity at 100 steps:", sens)
-    d, r = oracle_run("c2", mk, prm, 100, tslb.F64)
-    e = errs(gpu_run(d, prm, 100, tslb.F64, kernel), r)
-    print("c2", KNAME[kernel], "f64 100", e)
-    for k, v in e.items():
-        assert v <= max(1e-12, 10 * sens[k]), (k, v, sens[k])
+    gold = _golden_c2_conditioning()
+    d = round_inputs(inputs.static_droplet(64, 16.0, 4.0), tslb.F64)
+    o = ref.Oracle(64, 64, 64, 1.0, **oracle_kwargs(prm))
+    o.init_fields(d["rho"], d["ux"], d["uy"], d["uz"], d["phi"])
+    g = tslb.Tslb(64, 64, 64, 1.0, precision=tslb.F64, kernel=kernel, **gpu_kwargs(prm))
+    g.init_fields(d["rho"], d["ux"], d["uy"], d["uz"], d["phi"])
+    t = 0
+    for steps in (10, 30, 50, 100):
+        o.step(steps - t)
+        g.step(steps - t)
+        t = steps
+        m = {k: (None if v is None else np.asarray(v, dtype=np.float64)) for k, v in g.get_moments().items()}
+        e = errs(m, o.get_moments())
+        print("c2", KNAME[kernel], "f64 step", steps, {k: "%.2e" % v for k, v in e.items()},
+              "in units of the oracle's one-ulp drift:", {k: "%.2f" % (v / gold[steps][k]) for k, v in e.items()})
+        for k, v in e.items():
+            tol = 1e-12 if steps == 10 else max(1e-12, C2_FACTOR * gold[steps][k])
+            assert v <= tol, (steps, k, v, tol)
+    o.close()
+    g.close()
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
