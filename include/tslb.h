@@ -97,19 +97,33 @@ typedef struct {
   int forcing;             /* TSLB_FORCING_KICK | TSLB_FORCING_GUO                             */
 } tslb_params;
 
-/* Device bytes the context needs: 2 x (10 moment arrays [+ phi]) in the padded internal layout
- * (x/y ghost cells for the periodic wrap).  0 if the parameters are invalid.     */
+/* Device bytes the context needs: 2 buffers (the paper's rule "read the fields of time t, write elsewhere",
+ * PAPER.md:94-96, 213, kept as double buffering) x (10 moment arrays rho, u, Pi^neq -- what the method
+ * stores per node, PAPER.md:108 -- [+ phi, PAPER.md:198-211]) in the padded internal layout (x/y ghost
+ * cells for the periodic wrap), plus scratch arrays of the generic kernel.  Host
+ * function, no device work.  0 if the parameters are invalid.                                       */
 size_t tslb_workspace_bytes(const tslb_params *p);
 
-/* Validate parameters, select the device, allocate (or adopt) the workspace, build the TMA
- * descriptors.  On failure *out is NULL and, if out_err is passed to tslb_last_error(NULL), the
- * message of the failed create is returned.                                                     */
+/* Create a context for the problem the paper states: grid, relaxation frequency
+ * omega <-> nu = c_s^2 (1/omega - 1/2), surface tension sigma (eq. 20),
+ * interface width, boundary types (eqs. 9-10, 223).  Validates the
+ * parameters (TSLB_EINVAL: sizes <= 0, omega outside (0,2), sigma < 0 or not finite, W <= 0 when
+ * two_component, |jet_velocity| >= 1, jet_perturbation outside [0,1], nz < 4 with inflow/outflow,
+ * unsupported face pair, kernel/forcing combination), selects the device (TSLB_ECUDA when there is no
+ * sm_100 device: no CPU fallback), allocates the workspace with cudaMalloc or adopts the caller's
+ * (TSLB_ENOMEM / TSLB_EINVAL), builds the TMA descriptors of the tiled kernel.  On failure *out is NULL
+ * and tslb_last_error(NULL) returns the message of the failed create (per thread).  The context keeps
+ * `workspace` and `stream`; both must outlive it.                                                    */
 int tslb_create(const tslb_params *p, tslb_ctx **out);
 
-/* Set the time-0 state and reset the step counter.  rho, ux, uy, uz: required.  phi: required
- * iff two_component (else must be NULL).  pineq: NULL (-> Pi^neq = 0, a plain equilibrium start)
- * or 6 pointers xx,yy,zz,xy,xz,yz.  With inflow/outflow the two z boundary planes are then set
- * from the initial fields as in a step (hash step index 0).                                     */
+/* Set the time-0 state and reset the step counter.  The state IS the collision-ready moments of
+ * the first collision builds f^eq(rho, u) + (1 - omega) f^neq(Pi^neq, u) from them
+ * (eq. 5), so Pi^neq = 0 is a plain equilibrium start.  rho, ux, uy, uz: required.  phi:
+ * required iff two_component (else must be NULL; TSLB_EINVAL).  pineq: NULL (-> Pi^neq = 0) or 6
+ * pointers xx,yy,zz,xy,xz,yz (NULL entries -> 0).  With inflow/outflow the two z boundary planes are
+ * then set from the initial fields as in a step (eqs. 9-10, readings A10/A11; hash
+ * step index 0).  Copies the caller's arrays (host arrays through a pinned-free staging buffer);
+ * synchronises the stream.                                                                           */
 int tslb_init_fields(tslb_ctx *c, const void *rho, const void *ux, const void *uy, const void *uz,
                      const void *phi, const void *const pineq[6], int pointers_on_device);
 
@@ -117,7 +131,8 @@ int tslb_init_fields(tslb_ctx *c, const void *rho, const void *ux, const void *u
  * the context's stream.  TSLB_ESTATE before tslb_init_fields.                                   */
 int tslb_step(tslb_ctx *c, int nsteps);
 
-/* Copy out the stored state: rho, the stored velocity (KICK: the post-kick u'; GUO: the bare u_b;
+/* Copy out the stored state -- the moments the method keeps per node and phi
+ * (PAPER.md:198-211): rho, the stored velocity (KICK: the post-kick u'; GUO: the bare u_b;
  * see tslb_get_physical_velocity), Pi^neq (NOT the full Pi; reading A2; relative to u_b) and phi.  Any
  * pointer (and any entry of pineq, or pineq itself) may be NULL.  Synchronises the stream.      */
 int tslb_get_moments(tslb_ctx *c, void *rho, void *ux, void *uy, void *uz, void *const pineq[6],
@@ -179,6 +194,12 @@ int tslb_attach_neighbor(tslb_ctx *c, int face, void *nb_workspace, int nb_nz);
 int tslb_ipc_get_handle(tslb_ctx *c, void *handle64);
 int tslb_attach_neighbor_ipc(tslb_ctx *c, int face, const void *handle64, int nb_nz);
 
+/* Forget the attached neighbours (synchronises the stream; closes handles opened by
+ * tslb_attach_neighbor_ipc).  Tear-down across processes is two-phase: every rank detaches, a
+ * barrier, then every rank destroys -- CUDA forbids freeing exported memory that an importer still
+ * has open.  tslb_step on a detached halo face fails with TSLB_ESTATE.                             */
+int tslb_detach_neighbors(tslb_ctx *c);
+
 /* Copy the face planes of the CURRENT buffer into the attached neighbours' ghost planes
  * (asynchronous on the stream).  Needed once after tslb_init_fields; afterwards tslb_step keeps
  * the ghost planes current by itself.                                                           */
@@ -209,6 +230,8 @@ long long tslb_launch_count(const tslb_ctx *c);
  * y in [0,ny) into out[nx*ny] doubles (host pointer) -- test probe for the bit-exact hash pin.  */
 int tslb_debug_xi(tslb_ctx *c, long long step, double *out_host);
 
+/* Synchronise the stream, close imported neighbour handles, free what the library allocated (not a
+ * caller-owned workspace).  NULL is accepted.  Always TSLB_OK.                                      */
 int tslb_destroy(tslb_ctx *c);
 
 /* Last error message of the context (or of the last failed tslb_create when c == NULL).

@@ -80,11 +80,18 @@ Validated validate(const tslb_params *p) {
     if (!(v.halo_lo || v.jet_lo) || !(v.halo_hi || v.out_hi))
       return fail("a slab face is TSLB_BC_HALO, or JET_INFLOW (z low) / OUTFLOW (z high)");
     if (p->nz < 2) return fail("a slab needs nz >= 2 (the halo is two planes deep)");
+    // the imposed plane is not pushed to the neighbour: with nz == 2 it would be the neighbour's second
+    // ghost plane of phi, which would go stale
+    if ((v.jet_lo || v.out_hi) && p->nz < 3) return fail("a slab with an inflow or outflow face needs nz >= 3");
   } else {
     if (!zper && !jet) return fail("boundary types must be PERIODIC/PERIODIC or JET_INFLOW/OUTFLOW (or TSLB_BC_HALO faces)");
     if (jet && p->nz < 4) return fail("nz >= 4 is required with inflow/outflow");
   }
-  if ((v.jet_lo || v.out_hi) && !(p->jet_diameter >= 0.0)) return fail("jet_diameter must be >= 0");
+  if ((v.jet_lo || v.out_hi) && !(p->jet_diameter >= 0.0 && p->jet_diameter < 1e9)) return fail("jet_diameter must be finite and >= 0");
+  if (!(p->sigma >= 0.0 && p->sigma < 1e30)) return fail("sigma must be finite and >= 0");
+  if (!(p->jet_velocity > -1.0 && p->jet_velocity < 1.0)) return fail("jet_velocity must be finite and |U| < 1 (lattice units)");
+  if (!(p->jet_perturbation >= 0.0 && p->jet_perturbation <= 1.0)) return fail("jet_perturbation must be in [0, 1]");
+  if (p->two_component && !(p->interface_width < 1e9)) return fail("interface_width must be finite");
   if (p->kernel < TSLB_KERNEL_AUTO || p->kernel > TSLB_KERNEL_TILED) return fail("unknown kernel selector");
   if (p->forcing != TSLB_FORCING_KICK && p->forcing != TSLB_FORCING_GUO) return fail("unknown forcing selector");
   const bool guo = p->forcing == TSLB_FORCING_GUO;
@@ -632,6 +639,18 @@ int tslb_attach_neighbor_ipc(tslb_ctx *c, int face, const void *handle64, int nb
   if (c->nb_ipc[face]) cudaIpcCloseMemHandle(c->nb_ipc[face]);
   c->nb_ipc[face] = base;
   memcpy(c->nb_handle[face], handle64, 64);
+  return TSLB_OK;
+}
+
+int tslb_detach_neighbors(tslb_ctx *c) {
+  if (!c) return TSLB_EINVAL;
+  CK(cudaSetDevice(c->p.device));
+  CK(cudaStreamSynchronize(c->stream));
+  void *a = c->nb_ipc[0], *b = c->nb_ipc[1];
+  if (a) CK(cudaIpcCloseMemHandle(a));
+  if (b && b != a) CK(cudaIpcCloseMemHandle(b));
+  c->nb_ipc[0] = c->nb_ipc[1] = nullptr;
+  c->nb_on[0] = c->nb_on[1] = false;
   return TSLB_OK;
 }
 

@@ -26,12 +26,6 @@ template <> struct __align__(16) Pair<double> {
 typedef Pair<float> F2;
 typedef Pair<double> D2;
 
-#ifdef TSLB_SCALAR_PAIR
-__device__ __forceinline__ F2 operator+(F2 a, F2 b) { return F2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ F2 operator-(F2 a, F2 b) { return F2(a.x - b.x, a.y - b.y); }
-__device__ __forceinline__ F2 operator*(F2 a, F2 b) { return F2(a.x * b.x, a.y * b.y); }
-__device__ __forceinline__ F2 pfma(F2 a, F2 b, F2 c) { return F2(fmaf(a.x, b.x, c.x), fmaf(a.y, b.y, c.y)); }
-#else
 __device__ __forceinline__ F2 operator+(F2 a, F2 b) {
   float2 r = __fadd2_rn(make_float2(a.x, a.y), make_float2(b.x, b.y));
   return F2(r.x, r.y);
@@ -49,7 +43,6 @@ __device__ __forceinline__ F2 pfma(F2 a, F2 b, F2 c) {
   float2 r = __ffma2_rn(make_float2(a.x, a.y), make_float2(b.x, b.y), make_float2(c.x, c.y));
   return F2(r.x, r.y);
 }
-#endif
 // a*s + c with a broadcast scalar
 __device__ __forceinline__ F2 pfma(F2 a, float s, F2 c) { return pfma(a, F2(s), c); }
 __device__ __forceinline__ F2 operator*(F2 a, float s) { return a * F2(s); }

@@ -773,18 +773,11 @@ struct TiledPlan {
 
 // tile shapes: 32x8 in both precisions (fp32: ~103 KB of shared memory -> two CTAs per SM, whose
 // barrier phases interleave; measured 30.2 vs 27.6 GLUPS for 64x8 on C5)
-#ifndef TSLB_F32_TX
-#define TSLB_F32_TX 32
-#endif
-#ifndef TSLB_F64_TX
-#define TSLB_F64_TX 32
-#endif
-#ifndef TSLB_TY
-#define TSLB_TY 8
-#endif
+constexpr int TILE_TX = 32, TILE_TY = 8;
 inline void tiled_tile(int precision, int &tx, int &ty) {
-  tx = precision == TSLB_F32 ? TSLB_F32_TX : TSLB_F64_TX;
-  ty = TSLB_TY;
+  (void)precision;
+  tx = TILE_TX;
+  ty = TILE_TY;
 }
 
 inline bool tiled_supported(int precision, int nx, int ny, int nz) {
@@ -845,7 +838,6 @@ inline bool tiled_plan_create(TiledPlan &pl, int precision, const Layout &L, voi
     const long long cost = ((ctas + slots - 1) / slots) * (c + 5);
     if (best < 0 || cost < best) { best = cost; zc = c; }
   }
-  if (const char *env = getenv("TSLB_ZCHUNK")) { int v = atoi(env); if (v > 0) zc = v; }
   pl.zc = zc;
   pl.maps[0].zc = pl.maps[1].zc = zc;
   pl.name = "tiled<" + std::to_string(pl.tx) + "x" + std::to_string(pl.ty) + ",zc=" + std::to_string(zc) + ">";
@@ -912,11 +904,11 @@ template <typename T>
 cudaError_t launch_tiled(TiledPlan &pl, const StepParams<T> &P, int src, int order, bool two, cudaStream_t st);
 template <>
 inline cudaError_t launch_tiled<float>(TiledPlan &pl, const StepParams<float> &P, int src, int order, bool two, cudaStream_t st) {
-  return launch_tiled_t<float, TSLB_F32_TX, TSLB_TY>(pl, P, src, order, two, st);
+  return launch_tiled_t<float, TILE_TX, TILE_TY>(pl, P, src, order, two, st);
 }
 template <>
 inline cudaError_t launch_tiled<double>(TiledPlan &pl, const StepParams<double> &P, int src, int order, bool two, cudaStream_t st) {
-  return launch_tiled_t<double, TSLB_F64_TX, TSLB_TY>(pl, P, src, order, two, st);
+  return launch_tiled_t<double, TILE_TX, TILE_TY>(pl, P, src, order, two, st);
 }
 
 }  // namespace tslb

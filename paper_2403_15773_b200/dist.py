@@ -1,8 +1,9 @@
 """Multi-rank bookkeeping for the benchmark (torch.distributed plumbing only).
 
-The path does not shard yet ("replicas only"): every rank steps its own copy of the
-workload and there is no data-path collective.  What crosses ranks is the timing protocol of the
-bench contract: a barrier on both sides of the timed region, the MAX over ranks of the device
+The timing protocol of the bench contract, for both multi-GPU modes of bench.py: "replicas only" (the
+default: every rank steps its own copy of the workload, no data-path collective) and the z-slab
+decomposition of ONE domain (slabs.py; the halo planes are pushed by the step kernels themselves).
+What crosses ranks here: a barrier on both sides of the timed region, the MAX over ranks of the device
 time, and the whole-job throughput = units processed by all ranks / that time.
 Works with any backend (nccl on GPUs, gloo in the CPU tests).
 """

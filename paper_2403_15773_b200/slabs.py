@@ -13,10 +13,12 @@ import numpy as np
 from . import tslb
 
 
-def slab_ranges(nz, n):
-    """Balanced contiguous split of planes 0..nz-1 into n slabs -> [(z0, z1), ...] (z1 exclusive)."""
-    if n < 1 or nz < 2 * n:
-        raise ValueError("need at least two planes per slab: nz=%d, slabs=%d" % (nz, n))
+def slab_ranges(nz, n, jet=False):
+    """Balanced contiguous split of planes 0..nz-1 into n slabs -> [(z0, z1), ...] (z1 exclusive).
+    Two planes per slab at least (the halo is two planes deep); three where a slab carries the inflow or
+    the outflow plane (that plane is imposed, not pushed to the neighbour)."""
+    if n < 1 or nz < 2 * n or (jet and n > 1 and nz // n < 3):
+        raise ValueError("too few planes per slab: nz=%d, slabs=%d" % (nz, n))
     base, rem = divmod(nz, n)
     out, z = [], 0
     for r in range(n):
@@ -51,7 +53,7 @@ class LocalSlabs:
 
     def __init__(self, nx, ny, nz, omega, n_slabs, precision=tslb.F32, devices=None, jet=False, **kw):
         self.shape = (nz, ny, nx)
-        self.ranges = slab_ranges(nz, n_slabs)
+        self.ranges = slab_ranges(nz, n_slabs, jet)
         self.devices = list(devices) if devices is not None else [0] * n_slabs
         self.plans = [neighbor_plan(r, n_slabs, jet) for r in range(n_slabs)]
         self.sims = []
@@ -138,7 +140,7 @@ class RankSlab:
         import torch.distributed as dist
         self._torch, self._dist = torch, dist
         self.rank, self.world = dist.get_rank(), dist.get_world_size()
-        self.ranges = slab_ranges(nz, self.world)
+        self.ranges = slab_ranges(nz, self.world, jet)
         self.z0, self.z1 = self.ranges[self.rank]
         self.plan = neighbor_plan(self.rank, self.world, jet)
         self.device = device
@@ -181,7 +183,10 @@ class RankSlab:
         return self.sim.get_moments(**kw)
 
     def close(self):
+        """Two phases: every rank closes the handles it imported, a barrier, then every rank frees its own
+        workspace (freeing exported memory that an importer still has open is undefined behaviour)."""
         self._torch.cuda.synchronize(self.device)
+        self.sim.detach_neighbors()
         if self.world > 1:
-            self._dist.barrier()                       # neighbours may still hold my handle
+            self._dist.barrier()
         self.sim.close()

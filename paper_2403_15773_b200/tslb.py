@@ -22,7 +22,7 @@ EXPORTS = ["tslb_workspace_bytes", "tslb_create", "tslb_init_fields", "tslb_step
            "tslb_get_moments", "tslb_get_physical_velocity", "tslb_get_physical_velocity_noalloc",
            "tslb_noalloc_scratch_bytes", "tslb_step_count", "tslb_kernel_name", "tslb_launch_count",
            "tslb_debug_xi", "tslb_destroy", "tslb_last_error", "tslb_workspace_ptr",
-           "tslb_attach_neighbor", "tslb_ipc_get_handle", "tslb_attach_neighbor_ipc", "tslb_halo_push",
+           "tslb_attach_neighbor", "tslb_ipc_get_handle", "tslb_attach_neighbor_ipc", "tslb_detach_neighbors", "tslb_halo_push",
            "tslb_stats_begin", "tslb_stats_get", "tslb_stats_end"]
 
 
@@ -88,6 +88,7 @@ def lib():
         L.tslb_attach_neighbor.argtypes = [vp, ctypes.c_int, vp, ctypes.c_int]
         L.tslb_ipc_get_handle.argtypes = [vp, vp]
         L.tslb_attach_neighbor_ipc.argtypes = [vp, ctypes.c_int, vp, ctypes.c_int]
+        L.tslb_detach_neighbors.argtypes = [vp]
         L.tslb_halo_push.argtypes = [vp]
         L.tslb_stats_begin.argtypes = [vp, ctypes.c_int]
         L.tslb_stats_get.argtypes = [vp, vp, vp, ctypes.POINTER(ctypes.c_longlong)]
@@ -266,6 +267,9 @@ class Tslb:
     def attach_neighbor_ipc(self, face, handle, nb_nz):
         buf = ctypes.create_string_buffer(bytes(handle), 64)
         self._check(lib().tslb_attach_neighbor_ipc(self._h, int(face), buf, int(nb_nz)))
+
+    def detach_neighbors(self):
+        self._check(lib().tslb_detach_neighbors(self._h))
 
     def halo_push(self):
         self._check(lib().tslb_halo_push(self._h))

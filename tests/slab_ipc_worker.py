@@ -1,6 +1,7 @@
-"""Worker of test_slabs_gpu.py::test_two_processes_cuda_ipc -- launched by torch.distributed.run
-with two ranks (gloo), both on GPU 0: each rank owns one z-slab (slabs.RankSlab), rank 0 gathers
-the result and writes it to the .npz given as argv[1]."""
+"""Worker of test_slabs_gpu.py::test_two_processes_cuda_ipc / test_two_ranks_two_gpus_nccl -- launched by
+torch.distributed.run with two ranks: each rank owns one z-slab (slabs.RankSlab), rank 0 gathers the
+result and writes it to the .npz given as argv[1].  argv[3] = "gloo" (default: both ranks on GPU 0, host
+barrier per step) or "nccl" (rank r on GPU r: peer stores over NVLink, one-element all-reduce per step)."""
 import sys
 
 import numpy as np
@@ -24,11 +25,19 @@ def case(jet):
 def main():
     import torch.distributed as dist
     from paper_2403_15773_b200 import slabs, tslb
+    import os
+    import torch
     out, jet = sys.argv[1], sys.argv[2] == "1"
-    dist.init_process_group("gloo")
+    backend = sys.argv[3] if len(sys.argv) > 3 else "gloo"
+    device = int(os.environ.get("LOCAL_RANK", "0")) if backend == "nccl" else 0
+    torch.cuda.set_device(device)
+    if backend == "nccl":
+        dist.init_process_group("nccl", device_id=torch.device("cuda", device))
+    else:
+        dist.init_process_group("gloo")
     d, prm = case(jet)
     kw = {k: v for k, v in prm.items() if k not in ("nx", "ny", "nz", "omega")}
-    s = slabs.RankSlab(prm["nx"], prm["ny"], prm["nz"], prm["omega"], precision=tslb.F32, device=0, **kw)
+    s = slabs.RankSlab(prm["nx"], prm["ny"], prm["nz"], prm["omega"], precision=tslb.F32, device=device, **kw)
     z0, z1 = s.z0, s.z1
     pq = None if d.get("pineq") is None else [np.ascontiguousarray(a[z0:z1]) for a in d["pineq"]]
     s.init_fields(*[np.ascontiguousarray(d[k][z0:z1]) for k in ("rho", "ux", "uy", "uz")],

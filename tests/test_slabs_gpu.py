@@ -140,3 +140,57 @@ def test_two_processes_cuda_ipc(tmp_path, jet):
     one, _ = run_single(d, prm, w.STEPS, tslb.F32, tslb.KERNEL_AUTO)
     for k in ("rho", "ux", "uy", "uz", "phi", "pineq"):
         assert np.array_equal(z[k], one[k]), k
+
+
+# ---------------------------------------------------------------- more than one GPU (skipped on a 1-GPU box)
+def _need_two_gpus():
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+
+
+@pytest.mark.parametrize("kernel", [tslb.KERNEL_TILED, tslb.KERNEL_GENERIC])
+@pytest.mark.parametrize("jet", [False, True])
+def test_local_slabs_on_two_devices(kernel, jet):
+    """One process, slabs on devices 0 and 1: peer-mapped stores into the neighbour's ghost planes; the
+    tiled kernel's dynamic shared-memory attribute has to be set on EACH device."""
+    _need_two_gpus()
+    from tests import slab_ipc_worker as w
+    d, prm = w.case(jet)
+    one, _ = run_single(d, prm, w.STEPS, tslb.F32, kernel)
+    s = slabs.LocalSlabs(prm["nx"], prm["ny"], prm["nz"], prm["omega"], 2, precision=tslb.F32, devices=[0, 1],
+                         kernel=kernel, **gpu_kwargs(prm))
+    s.init_fields(d["rho"], d["ux"], d["uy"], d["uz"], d.get("phi"), d.get("pineq"))
+    s.step(w.STEPS)
+    many = s.get_moments()
+    s.close()
+    same_bits(one, many)
+
+
+@pytest.mark.parametrize("jet", [False, True])
+def test_two_ranks_two_gpus_nccl(tmp_path, jet):
+    """One process per GPU (RankSlab): CUDA IPC handles, peer stores across devices, and the per-step
+    barrier as a one-element NCCL all-reduce on the library's stream."""
+    _need_two_gpus()
+    out = str(tmp_path / "nccl.npz")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2", "--master-addr",
+           "127.0.0.1", "--master-port", "29519", os.path.join(ROOT, "tests", "slab_ipc_worker.py"), out,
+           "1" if jet else "0", "nccl"]
+    env = dict(os.environ, PYTHONPATH=ROOT + os.pathsep + os.environ.get("PYTHONPATH", ""))
+    r = subprocess.run(cmd, cwd=ROOT, env=env, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-4000:]
+    z = np.load(out)
+    from tests import slab_ipc_worker as w
+    d, prm = w.case(jet)
+    one, _ = run_single(d, prm, w.STEPS, tslb.F32, tslb.KERNEL_AUTO)
+    for k in ("rho", "ux", "uy", "uz", "phi", "pineq"):
+        assert np.array_equal(z[k], one[k]), k
+
+
+def test_slab_with_an_imposed_plane_needs_three_planes():
+    with pytest.raises(tslb.TslbError, match="nz >= 3"):
+        tslb.Tslb(32, 8, 2, 1.0, two_component=True, sigma=0.01, bc_zlo=tslb.BC_JET_INFLOW, bc_zhi=tslb.BC_HALO,
+                  jet_diameter=4.0, jet_velocity=0.05)
+    with pytest.raises(ValueError):
+        slabs.slab_ranges(8, 4, jet=True)
+    assert slabs.slab_ranges(12, 4, jet=True) == [(0, 3), (3, 6), (6, 9), (9, 12)]
