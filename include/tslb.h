@@ -128,7 +128,11 @@ int tslb_init_fields(tslb_ctx *c, const void *rho, const void *ux, const void *u
                      const void *phi, const void *const pineq[6], int pointers_on_device);
 
 /* Advance nsteps >= 0 time steps (eq. 6 + 206 eq. 23 per step).  Asynchronous on
- * the context's stream.  TSLB_ESTATE before tslb_init_fields.                                   */
+ * the context's stream.  TSLB_ESTATE before tslb_init_fields.  From nsteps = 5 on (and on a stream
+ * other than the legacy default stream) the steps are replayed from a CUDA graph of two steps that the
+ * context captures once per starting buffer, so that small grids are not bound by kernel launches;
+ * the first such call allocates an 8-byte device counter.  Do not call it with nsteps >= 5 while the
+ * stream is itself being captured.                                                                  */
 int tslb_step(tslb_ctx *c, int nsteps);
 
 /* Copy out the stored state -- the moments the method keeps per node and phi

@@ -138,11 +138,20 @@ struct tslb_ctx {
   bool inited = false;
   long long t = 0;
   long long launches = 0;
-  void *stage = nullptr;       // one dense field, for host <-> device import/export
+  void *stage[2] = {nullptr, nullptr};   // two dense fields, for host <-> device import/export: the copy of one
+                                          // field overlaps the (un)packing of the other
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
+  void *pv_tmp = nullptr;      // tslb_get_physical_velocity to host pointers: three dense fields, kept
   double *stat = nullptr;      // mid-plane running sums: [0] phi, [1] u_z, nx*nz doubles each
   int stat_every = 0;          // 0: off
   long long stat_n = 0;        // samples accumulated
   TiledPlan tiled;             // TMA descriptors etc.
+  // tslb_step(n) as a replayed CUDA graph of two steps (buffer 0 -> 1 -> 0 or 1 -> 0 -> 1); the kernels read
+  // the step index from step_ctr, which a one-thread kernel advances before every step
+  cudaGraphExec_t gexec[2] = {nullptr, nullptr};
+  long long *step_ctr = nullptr;
+  bool graph_failed = false;
   std::string err;
   std::string kname;
 
@@ -192,6 +201,7 @@ StepParams<T> make_step_params(tslb_ctx *c, int src, int dst) {
   P.jetP = (T)c->p.jet_perturbation;
   P.seed = c->p.seed;
   P.step_next = c->t + 1;
+  P.step_ctr = nullptr;
   return P;
 }
 
@@ -224,18 +234,54 @@ int launch_generic(tslb_ctx *c, const StepParams<T> &P) {
   return TSLB_OK;
 }
 
+__global__ void step_ctr_set_kernel(long long *ctr, long long v) { *ctr = v; }
+__global__ void step_ctr_tick_kernel(long long *ctr) { *ctr += 1; }
+
+// one time step src -> dst on the stream (no bookkeeping); step_ctr != null: graph capture
+template <typename T>
+int launch_step(tslb_ctx *c, int src, const long long *step_ctr) {
+  StepParams<T> P = make_step_params<T>(c, src, src ^ 1);
+  P.step_ctr = step_ctr;
+  if (c->v.kernel == TSLB_KERNEL_TILED) {
+    cudaError_t e = launch_tiled<T>(c->tiled, P, src, c->p.hermite_order, c->p.two_component != 0, c->stream);
+    c->launches += (c->v.jet_lo || c->v.out_hi) ? 2 : 1;   // + the boundary-plane kernel with inflow/outflow
+    return e == cudaSuccess ? TSLB_OK : c->cuda_fail(e, "launch_tiled");
+  }
+  return launch_generic<T>(c, P);
+}
+
+// Build (once per starting buffer) the graph of two steps cur -> cur^1 -> cur by stream capture.
+template <typename T>
+bool graph_build(tslb_ctx *c, int cur) {
+  if (c->gexec[cur]) return true;
+  if (c->graph_failed || !c->stream) return false;          // the legacy default stream cannot be captured
+  if (!c->step_ctr && cudaMalloc((void **)&c->step_ctr, sizeof(long long)) != cudaSuccess) {
+    cudaGetLastError();
+    c->graph_failed = true;
+    return false;
+  }
+  const long long keep = c->launches;
+  cudaGraph_t g = nullptr;
+  bool ok = cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+  if (ok) {
+    for (int h = 0; h < 2 && ok; ++h) {
+      step_ctr_tick_kernel<<<1, 1, 0, c->stream>>>(c->step_ctr);
+      ok = launch_step<T>(c, cur ^ h, c->step_ctr) == TSLB_OK;
+    }
+    ok = (cudaStreamEndCapture(c->stream, &g) == cudaSuccess) && ok && g;
+  }
+  if (ok) ok = cudaGraphInstantiate(&c->gexec[cur], g, 0) == cudaSuccess;
+  if (g) cudaGraphDestroy(g);
+  c->launches = keep;
+  if (!ok) { cudaGetLastError(); c->gexec[cur] = nullptr; c->graph_failed = true; }
+  return ok;
+}
+
 template <typename T>
 int step_typed(tslb_ctx *c, int nsteps) {
-  for (int s = 0; s < nsteps; ++s) {
-    StepParams<T> P = make_step_params<T>(c, c->cur, c->cur ^ 1);
-    int rc;
-    if (c->v.kernel == TSLB_KERNEL_TILED) {
-      cudaError_t e = launch_tiled<T>(c->tiled, P, c->cur, c->p.hermite_order, c->p.two_component != 0, c->stream);
-      c->launches += (c->v.jet_lo || c->v.out_hi) ? 2 : 1;   // + the boundary-plane kernel with inflow/outflow
-      rc = (e == cudaSuccess) ? TSLB_OK : c->cuda_fail(e, "launch_tiled");
-    } else {
-      rc = launch_generic<T>(c, P);
-    }
+  // one step launched from the host, with its bookkeeping
+  auto one_step = [&]() -> int {
+    int rc = launch_step<T>(c, c->cur, nullptr);
     if (rc != TSLB_OK) return rc;
     c->cur ^= 1;
     c->t++;
@@ -250,6 +296,32 @@ int step_typed(tslb_ctx *c, int nsteps) {
       c->launches++;
       c->stat_n++;
     }
+    return TSLB_OK;
+  };
+  // Many short steps (small grids): replay a captured graph of two steps instead of launching 2-3 kernels per
+  // step from the host.  Not for slabs (one step per call) nor while the mid-plane statistics are sampled.  The
+  // first step of a context is launched directly (it sets the kernel attributes, which a capture must not).
+  if (nsteps >= 5 && !c->v.slab && !c->stat_every && c->stream && !c->graph_failed) {
+    if (c->launches == 0) {
+      int rc = one_step();
+      if (rc != TSLB_OK) return rc;
+      --nsteps;
+    }
+    if (graph_build<T>(c, c->cur)) {
+      const int pairs = nsteps / 2;
+      const long long per_step = c->v.kernel == TSLB_KERNEL_TILED ? ((c->v.jet_lo || c->v.out_hi) ? 2 : 1)
+                                 : (c->p.two_component ? (c->p.forcing == TSLB_FORCING_GUO ? 3 : 2) : 1);
+      step_ctr_set_kernel<<<1, 1, 0, c->stream>>>(c->step_ctr, c->t);
+      for (int g = 0; g < pairs; ++g) CK(cudaGraphLaunch(c->gexec[c->cur], c->stream));
+      CK(cudaGetLastError());
+      c->t += 2LL * pairs;
+      c->launches += 2LL * pairs * (per_step + 1) + 1;      // + the one-thread counter kernels
+      nsteps -= 2 * pairs;
+    }
+  }
+  for (int s = 0; s < nsteps; ++s) {
+    int rc = one_step();
+    if (rc != TSLB_OK) return rc;
   }
   return TSLB_OK;
 }
@@ -283,9 +355,12 @@ int physvel_typed(tslb_ctx *c, void *const dst[3], int on_device) {
   for (int k = 0; k < NF_MAX; ++k) vel.f[k] = (T *)c->fields[c->cur][k];
   // host destinations: the three components go through scratch device memory of their own
   T *dev[3] = {nullptr, nullptr, nullptr};
-  T *tmp = nullptr;
   if (!on_device) {
-    CK(cudaMalloc((void **)&tmp, 3 * N * sizeof(T)));
+    if (!c->pv_tmp) {
+      cudaError_t e = cudaMalloc(&c->pv_tmp, 3 * N * sizeof(T));
+      if (e != cudaSuccess) return c->fail(TSLB_ENOMEM, "cudaMalloc(physical velocity): %s", cudaGetErrorString(e));
+    }
+    T *tmp = (T *)c->pv_tmp;
     for (int a = 0; a < 3; ++a) dev[a] = dst[a] ? tmp + a * N : nullptr;
   } else {
     for (int a = 0; a < 3; ++a) dev[a] = (T *)dst[a];
@@ -297,8 +372,23 @@ int physvel_typed(tslb_ctx *c, void *const dst[3], int on_device) {
     for (int a = 0; a < 3 && e == cudaSuccess; ++a)
       if (dst[a]) e = cudaMemcpyAsync(dst[a], dev[a], N * sizeof(T), cudaMemcpyDeviceToHost, c->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-  if (tmp) cudaFree(tmp);
   if (e != cudaSuccess) return c->cuda_fail(e, "tslb_get_physical_velocity");
+  return TSLB_OK;
+}
+
+// staging for host pointers: two device buffers of one dense field each, a copy stream and the events that
+// hand a buffer back and forth between the copy stream and the context's stream
+int stage_setup(tslb_ctx *c) {
+  const size_t N = (size_t)c->p.nx * c->p.ny * c->p.nz;
+  for (int b = 0; b < 2; ++b) {
+    if (!c->stage[b]) {
+      cudaError_t e = cudaMalloc(&c->stage[b], N * c->v.esize);
+      if (e != cudaSuccess) return c->fail(TSLB_ENOMEM, "cudaMalloc(stage): %s", cudaGetErrorString(e));
+    }
+    if (!c->ev_copied[b]) CK(cudaEventCreateWithFlags(&c->ev_copied[b], cudaEventDisableTiming));
+    if (!c->ev_free[b]) CK(cudaEventCreateWithFlags(&c->ev_free[b], cudaEventDisableTiming));
+  }
+  if (!c->copy_stream) CK(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
   return TSLB_OK;
 }
 
@@ -316,19 +406,27 @@ int init_typed(tslb_ctx *c, const void *const src[NF_MAX], int on_device) {
   const Layout &L = c->v.L;
   const size_t N = (size_t)L.nx * L.ny * L.nz;
   dim3 b(128), g((L.nx + 127) / 128, L.ny, L.nz);
+  // host arrays: field k is copied into one stage on the copy stream while the context's stream packs the
+  // previous field out of the other stage
+  if (!on_device) CK(cudaStreamSynchronize(c->stream));       // (the copy stream does not wait for earlier work)
+  int nh = 0;
   for (int k = 0; k < c->v.nfields; ++k) {
     const T *d = nullptr;
     if (src[k]) {
       if (on_device) {
         d = (const T *)src[k];
       } else {
-        CK(cudaMemcpyAsync(c->stage, src[k], N * sizeof(T), cudaMemcpyHostToDevice, c->stream));
-        d = (const T *)c->stage;
+        const int sb = nh++ & 1;
+        if (nh > 2) CK(cudaStreamWaitEvent(c->copy_stream, c->ev_free[sb], 0));
+        CK(cudaMemcpyAsync(c->stage[sb], src[k], N * sizeof(T), cudaMemcpyHostToDevice, c->copy_stream));
+        CK(cudaEventRecord(c->ev_copied[sb], c->copy_stream));
+        CK(cudaStreamWaitEvent(c->stream, c->ev_copied[sb], 0));
+        d = (const T *)c->stage[sb];
       }
     }
     pack_in_kernel<T><<<g, b, 0, c->stream>>>(L, d, (T *)c->fields[0][k], k == F_DRHO, d == nullptr);
     CK(cudaGetLastError());
-    if (!on_device && src[k]) CK(cudaStreamSynchronize(c->stream));   // stage is reused
+    if (!on_device && src[k]) CK(cudaEventRecord(c->ev_free[(nh - 1) & 1], c->stream));
   }
   c->cur = 0;
   c->t = 0;
@@ -358,16 +456,25 @@ int get_typed(tslb_ctx *c, void *const dst[NF_MAX], int on_device) {
   const Layout &L = c->v.L;
   const size_t N = (size_t)L.nx * L.ny * L.nz;
   dim3 b(128), g((L.nx + 127) / 128, L.ny, L.nz);
+  int nh = 0;
   for (int k = 0; k < c->v.nfields; ++k) {
     if (!dst[k]) continue;
-    T *d = on_device ? (T *)dst[k] : (T *)c->stage;
-    pack_out_kernel<T><<<g, b, 0, c->stream>>>(L, (const T *)c->fields[c->cur][k], d, k == F_DRHO);
-    CK(cudaGetLastError());
-    if (!on_device) {
-      CK(cudaMemcpyAsync(dst[k], c->stage, N * sizeof(T), cudaMemcpyDeviceToHost, c->stream));
-      CK(cudaStreamSynchronize(c->stream));
+    if (on_device) {
+      pack_out_kernel<T><<<g, b, 0, c->stream>>>(L, (const T *)c->fields[c->cur][k], (T *)dst[k], k == F_DRHO);
+      CK(cudaGetLastError());
+      continue;
     }
+    // host arrays: the context's stream unpacks field k into one stage while the copy stream sends the other out
+    const int sb = nh++ & 1;
+    if (nh > 2) CK(cudaStreamWaitEvent(c->stream, c->ev_free[sb], 0));
+    pack_out_kernel<T><<<g, b, 0, c->stream>>>(L, (const T *)c->fields[c->cur][k], (T *)c->stage[sb], k == F_DRHO);
+    CK(cudaGetLastError());
+    CK(cudaEventRecord(c->ev_copied[sb], c->stream));
+    CK(cudaStreamWaitEvent(c->copy_stream, c->ev_copied[sb], 0));
+    CK(cudaMemcpyAsync(dst[k], c->stage[sb], N * sizeof(T), cudaMemcpyDeviceToHost, c->copy_stream));
+    CK(cudaEventRecord(c->ev_free[sb], c->copy_stream));
   }
+  if (nh) CK(cudaStreamSynchronize(c->copy_stream));
   CK(cudaStreamSynchronize(c->stream));
   return TSLB_OK;
 }
@@ -511,10 +618,9 @@ int tslb_init_fields(tslb_ctx *c, const void *rho, const void *ux, const void *u
   if (c->p.two_component && !phi) return c->fail(TSLB_EINVAL, "phi is required when two_component");
   if (!c->p.two_component && phi) return c->fail(TSLB_EINVAL, "phi must be NULL when !two_component");
   CK(cudaSetDevice(c->p.device));
-  const size_t N = (size_t)c->p.nx * c->p.ny * c->p.nz;
-  if (!pointers_on_device && !c->stage) {
-    cudaError_t e = cudaMalloc(&c->stage, N * c->v.esize);
-    if (e != cudaSuccess) return c->fail(TSLB_ENOMEM, "cudaMalloc(stage): %s", cudaGetErrorString(e));
+  if (!pointers_on_device) {
+    int rc = stage_setup(c);
+    if (rc != TSLB_OK) return rc;
   }
   const void *src[NF_MAX] = {rho, ux, uy, uz, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, phi};
   if (pineq)
@@ -544,10 +650,9 @@ int tslb_get_moments(tslb_ctx *c, void *rho, void *ux, void *uy, void *uz, void 
   if (!c->inited) return c->fail(TSLB_ESTATE, "tslb_get_moments before tslb_init_fields");
   if (phi && !c->p.two_component) return c->fail(TSLB_EINVAL, "phi requested from a single-component context");
   CK(cudaSetDevice(c->p.device));
-  const size_t N = (size_t)c->p.nx * c->p.ny * c->p.nz;
-  if (!pointers_on_device && !c->stage) {
-    cudaError_t e = cudaMalloc(&c->stage, N * c->v.esize);
-    if (e != cudaSuccess) return c->fail(TSLB_ENOMEM, "cudaMalloc(stage): %s", cudaGetErrorString(e));
+  if (!pointers_on_device) {
+    int rc = stage_setup(c);
+    if (rc != TSLB_OK) return rc;
   }
   void *dst[NF_MAX] = {rho, ux, uy, uz, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, phi};
   if (pineq)
@@ -734,7 +839,16 @@ int tslb_destroy(tslb_ctx *c) {
   tiled_plan_destroy(c->tiled);
   for (int side = 0; side < 2; ++side)
     if (c->nb_ipc[side]) cudaIpcCloseMemHandle(c->nb_ipc[side]);
-  if (c->stage) cudaFree(c->stage);
+  for (int g = 0; g < 2; ++g)
+    if (c->gexec[g]) cudaGraphExecDestroy(c->gexec[g]);
+  if (c->step_ctr) cudaFree(c->step_ctr);
+  for (int b = 0; b < 2; ++b) {
+    if (c->stage[b]) cudaFree(c->stage[b]);
+    if (c->ev_copied[b]) cudaEventDestroy(c->ev_copied[b]);
+    if (c->ev_free[b]) cudaEventDestroy(c->ev_free[b]);
+  }
+  if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+  if (c->pv_tmp) cudaFree(c->pv_tmp);
   if (c->stat) cudaFree(c->stat);
   if (c->nrm_own) cudaFree(c->nrm_own);
   if (c->own_ws && c->ws) cudaFree(c->ws);

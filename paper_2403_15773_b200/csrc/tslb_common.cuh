@@ -63,7 +63,8 @@ struct StepParams {
   double jetD2;          // D^2, compared with (2x-(nx-1))^2 + (2y-(ny-1))^2
   T jetU, jetP;
   unsigned long long seed;
-  long long step_next;   // index t+1 of the step being computed (keys the hash)
+  long long step_next;   // index t+1 of the step being computed (keys the hash) ...
+  const long long *step_ctr;   // ... or, when not null (replayed CUDA graph), where to read it on the device
 };
 
 // Counter-based inflow perturbation (reading A12): splitmix64 finaliser of
@@ -87,6 +88,10 @@ template <typename T>
 __host__ __device__ inline T xi_value(unsigned long long seed, int x, int y, int nx, int ny, long long step) {
   return (T)xi_numerator(seed, x, y, nx, ny, step) * (T)(1.0 / 16777216.0);
 }
+
+// index t+1 of the step being computed
+template <typename T>
+__device__ __forceinline__ long long step_index(const StepParams<T> &P) { return P.step_ctr ? *P.step_ctr : P.step_next; }
 
 // source plane for a read at z, at most two planes outside [0, nz): ghost plane of a slab face,
 // periodic image, or the clamped boundary plane.  Branch-free: it sits in the hot loop of the tiled

@@ -167,7 +167,7 @@ __global__ void __launch_bounds__(128) generic_step_kernel(const __grid_constant
 
   if ((P.jet_lo && z == 0) || (P.out_hi && z == L.nz - 1)) {
     T o[NF_MAX];
-    boundary_node<T>(P, P.in, x, y, z, P.step_next, o, TWO);
+    boundary_node<T>(P, P.in, x, y, z, step_index(P), o, TWO);
 #pragma unroll
     for (int k = 0; k < NF; ++k) P.out.f[k][i0] = o[k];
     return;

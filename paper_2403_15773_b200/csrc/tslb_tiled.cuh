@@ -858,7 +858,7 @@ __global__ void tiled_boundary_kernel(const __grid_constant__ StepParams<T> P, i
   if (blockIdx.z ? !P.out_hi : !P.jet_lo) return;
   const int x = ((X - GX) % L.nx + L.nx) % L.nx, y = ((Y - GY) % L.ny + L.ny) % L.ny;
   T o[NF_MAX];
-  boundary_node<T>(P, P.in, x, y, z, P.step_next, o, two != 0);
+  boundary_node<T>(P, P.in, x, y, z, step_index(P), o, two != 0);
   const long long i0 = ((long long)z * L.py + Y) * L.px + X;
   const int nf = two ? 11 : 10;
   for (int k = 0; k < nf; ++k) P.out.f[k][i0] = o[k];

@@ -190,7 +190,7 @@ def test_two_ranks_two_gpus_nccl(tmp_path, jet):
 def test_slab_with_an_imposed_plane_needs_three_planes():
     with pytest.raises(tslb.TslbError, match="nz >= 3"):
         tslb.Tslb(32, 8, 2, 1.0, two_component=True, sigma=0.01, bc_zlo=tslb.BC_JET_INFLOW, bc_zhi=tslb.BC_HALO,
-                  jet_diameter=4.0, jet_velocity=0.05)
+                  jet_diameter=4.0, jet_velocity=0.05, torch_workspace=False)
     with pytest.raises(ValueError):
         slabs.slab_ranges(8, 4, jet=True)
     assert slabs.slab_ranges(12, 4, jet=True) == [(0, 3), (3, 6), (6, 9), (9, 12)]
