@@ -350,6 +350,10 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   const int kst = TWO ? z0 - 4 : z0 - 2;
   const int kfirst = TWO ? kst : z0 - 1; // first plane that has a TMA group
   const int NI = z1 - kst + 2;           // iterations: k = kst .. z1+1
+  // The same in iteration numbers i = k - kst (what the loops test: no plane arithmetic per iteration):
+  // plane z0 is iteration I0, plane z1 iteration IZ1.
+  constexpr int I0 = TWO ? 4 : 2;
+  const int IZ1 = I0 + (z1 - z0);
 
   // plane coordinate in the tensor map: wrapped / clamped / ghost plane of a slab (zsrc), shifted
   // by the ghost planes below z = 0
@@ -391,7 +395,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   // B: phase geometry and fluxes of one node pair (eqs. 20-24, readings A6-A8), iteration k.
   // ROLE 0: a tile pair (finishes and stores phi'); 1: a halo-row pair; 2: a halo-column pair.
   // bo / bn: element offsets of the exchange-block halves of plane parity k&1 / (k-1)&1.
-  auto phase_B = [&](auto role, auto drc, PhaseState<T> &st, const PairGeom &g0, int k, int s, int bo, int bn) {
+  auto phase_B = [&](auto role, auto drc, PhaseState<T> &st, const PairGeom &g0, int s, int bo, int bn) {
     constexpr int ROLE = decltype(role)::value, DR = decltype(drc)::value;   // DR: rows below the thread's first pair
     const PairGeom g = {g0.oP + DR * RX, g0.c0, g0.cl, g0.cr, g0.oZ + DR * ZW, g0.oF + DR * FQW, g0.oG + DR * TX, g0.oT + DR * TX};
     // in-plane combinations of phi(k+2) on rows r-1, r, r+1 (phi box rows r .. r+2): first along y on the
@@ -508,9 +512,9 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   uint32_t mph = TWO ? 0u : 1u;
   // end of an iteration: the ONE CTA barrier; in the halo-column warp (ISSUE) the group three planes ahead
   // goes into the slot just read
-  auto iter_end = [&](auto issues, int k) {
+  auto iter_end = [&](auto issues, int i) {
     __syncthreads();
-    if (decltype(issues)::value && issuer && k >= kfirst && has_group(k + S)) issue(k + S, s);
+    if (decltype(issues)::value && issuer && i >= I0 - (TWO ? 4 : 1) && i + S <= IZ1) issue(kst + i + S, s);
     s = s == S - 1 ? 0 : s + 1;
     if (s == 0) mph ^= 1u;
   };
@@ -529,10 +533,10 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   // extra row of the same field (+ RY for planes of odd parity)
   int oPL = lx == 0 ? TY * TX + r : oXP - 1, oPR = lx == LX - 1 ? TY * TX + r : oXM + 1;
   const int hpar = (lx == 0 ? 1 : 0) | (lx == LX - 1 ? 2 : 0);
-  auto xpass = [&](int k, int s, V (&A0)[9]) {
+  auto xpass = [&](bool odd, int s, V (&A0)[9]) {      // odd: parity of the plane
     const int oAM = oAP - 2 * TX;
     T *const xp = s_ap + oXP, *const xm = s_am + oXM;
-    const int hoff = (k & 1) * RY;
+    const int hoff = odd ? RY : 0;
     const T *pl = s_ap + oPL + ((hpar & 1) ? hoff : 0), *pr = s_am + oPR + ((hpar & 2) ? hoff : 0);
     V Xg[8][3];   // [group][p]
     {
@@ -586,6 +590,8 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     const int jlo = max(z0, P.jet_lo ? 1 : 0);
     const int njs = (gx_ >= xs && gy_ >= ys) ? min(z1, P.out_hi ? L.nz - 1 : L.nz) - jlo : 0;
     T *pst = P.out.f[0] + o00 + (long long)(kst - 2) * L.plane;   // field 0 of the pair, plane k-2
+    const int ju = kst - 2 - jlo;            // (plane k-2) - jlo = i + ju
+    bool odd = kst & 1;                      // parity of plane k; bo: its half of the exchange block
     // halo-row warp: D for the second pair of every phase thread (tile rows 3 + hi and 7 + hi)
     const int dZ = (3 + hi) * ZW + 2 + 2 * lx, dT = (2 + hi) * TX + 2 * lx;
     const int deoff = (lx == 0 ? C::B_ZL : (lx == LX - 1 ? C::B_ZL + RY : C::B_ZZ)) + 2 + 3 + hi;
@@ -594,25 +600,24 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     for (int i = 0; i < NI; ++i) {
       // (keep the loop-invariant offsets in registers: recomputing them from the thread index costs more)
       asm volatile("" : "+r"(oM), "+r"(oT), "+r"(oAP), "+r"(oXP), "+r"(oXM), "+r"(oPL), "+r"(oPR));
-      const int k = kst + i;
-      const int bo = (k & 1) * BUF;          // exchange-block half of this plane's parity
-      if (has_group(k)) mbar_wait(&bars[s], mph);
-      const bool src = k >= z0 - 1 && k <= z1;     // plane k is a source plane of this chunk
+      const int bo = odd ? BUF : 0;
+      if (i >= (TWO ? 0 : 1) && i <= IZ1) mbar_wait(&bars[s], mph);
+      const bool src = i >= I0 - 1 && i <= IZ1;    // plane k is a source plane of this chunk
       V A0[9];                               // own y-push term a0 per (c,p)
-      if (src) xpass(k, s, A0);
+      if (src) xpass(odd, s, A0);
       xpass_barrier();
-      if (TWO && halow && k <= z1 && k - 1 >= z0) {
+      if (TWO && halow && i <= IZ1 && i >= I0 + 1) {
         phase_D(IC<0>(), dZ, dT, s, BUF - bo, deoff, demask, design);
         phase_D(IC<4>(), dZ, dT, s, BUF - bo, deoff, demask, design);
       }
       V o[NF_MAX];
-      if (TWO && flow && (unsigned)(k - 2 - jlo) < (unsigned)njs) {
+      if (TWO && flow && (unsigned)(i + ju) < (unsigned)njs) {
         // a6: u'(k-2) = u_b + F / rho' with the F(k-2) the phase warps wrote in iteration k-1; a9: store it
         const T *kf = s_buf + bo + C::B_KF + oT;
         o[1] = pfma(lds_pair(kf), rinv, ubx);
         o[2] = pfma(lds_pair(kf + TLE), rinv, uby);
         o[3] = pfma(lds_pair(kf + 2 * TLE), rinv, ubz);
-        store_pair<T, FM_U, SLAB>(P, o, pst, k - 2, gx_, gy_, img0, fs);
+        store_pair<T, FM_U, SLAB>(P, o, pst, kst + i - 2, gx_, gy_, img0, fs);
       }
       if (flow && src) {
         // C: finish the y-pass of plane k (a+ from the row below, a- from the row above, own a0) and z-push
@@ -652,7 +657,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
         // a4: plane k-1 is complete: u_b = m'/rho', Pi^neq' = Pi' - rho' u_b u_b (Hermite form)
         rinv = prcp<T>(outm[0] + V(T(1)));
         ubx = outm[1] * rinv; uby = outm[2] * rinv; ubz = outm[3] * rinv;
-        if ((unsigned)(k - 1 - jlo) < (unsigned)njs) {
+        if ((unsigned)(i + ju + 1) < (unsigned)njs) {
           o[0] = outm[0];
           o[4] = outm[4] - outm[1] * ubx;
           o[5] = outm[5] - outm[2] * uby;
@@ -661,15 +666,16 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
           o[8] = outm[8] - outm[1] * ubz;
           o[9] = outm[9] - outm[2] * ubz;
           if (TWO) {
-            store_pair<T, FM_RHOPI, SLAB>(P, o, pst + L.plane, k - 1, gx_, gy_, img0, fs);
+            store_pair<T, FM_RHOPI, SLAB>(P, o, pst + L.plane, kst + i - 1, gx_, gy_, img0, fs);
           } else {
             o[1] = ubx; o[2] = uby; o[3] = ubz;
-            store_pair<T, FM_FLOW, SLAB>(P, o, pst + L.plane, k - 1, gx_, gy_, img0, fs);
+            store_pair<T, FM_FLOW, SLAB>(P, o, pst + L.plane, kst + i - 1, gx_, gy_, img0, fs);
           }
         }
       }
       pst += L.plane;
-      iter_end(IC<0>(), k);
+      odd = !odd;
+      iter_end(IC<0>(), i);
     }
   } else if (colw) {
     // ============================ halo-column warp ============================
@@ -680,11 +686,11 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     const int rh = hi ? 0 : RY - 1, ch = HL + 2 * lx;
     const PairGeom gc = {r * RX, c0, cl, cr, 0, r * FQW + (c0 - (HL - 2)) / 2, 0, 0};
     const PairGeom gh = {rh * RX, ch, ch - 1, ch + 2, rh * ZW + 2 + 2 * lx, rh * FQW + 1 + lx, rh * TX + 2 * lx, 0};
+    bool odd = kst & 1;                      // parity of plane k
     for (int i = 0; i < NI; ++i) {
-      const int k = kst + i;
-      const int bo = (k & 1) * BUF, bn = BUF - bo;
-      if (has_group(k)) mbar_wait(&bars[s], mph);
-      if (k + 1 >= z0 - 1 && k + 1 <= z1) {
+      const int bo = odd ? BUF : 0, bn = BUF - bo;
+      if (i >= (TWO ? 0 : 1) && i <= IZ1) mbar_wait(&bars[s], mph);
+      if (i >= I0 - 2 && i <= IZ1 - 1) {
         // x-pass terms of the two halo columns x0-1 (its a+) and x0+TX (its a-) of every region row of
         // plane k+1 (moments in the next ring slot), one iteration ahead of the rows that use them
         const int s1 = s == S - 1 ? 0 : s + 1;
@@ -704,16 +710,17 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
           push3<1, T, T>(K[K021], K[K021], K[K021], gp[5], gm[5], g0);
           push3<2, T, T>(K[K002], K[K102], K[K102], gp[6], gm[6], g0);
           push3<1, T, T>(K[K012], K[K012], K[K012], gp[7], gm[7], g0);
-          T *xh = (cside ? s_am : s_ap) + TY * TX + ((k + 1) & 1) * RY + r;
+          T *xh = (cside ? s_am : s_ap) + TY * TX + (odd ? 0 : RY) + r;      // parity of plane k+1
 #pragma unroll
           for (int g = 0; g < 8; ++g) xh[g * YPF] = cside ? gm[g] : gp[g];
         }
       }
-      if (TWO && k <= z1) {
-        if (lane < 2 * RY) phase_B(IC<2>(), IC<0>(), pc, gc, k, s, bo, bn);
-        phase_B(IC<1>(), IC<0>(), ph_, gh, k, s, bo, bn);
+      if (TWO && i <= IZ1) {
+        if (lane < 2 * RY) phase_B(IC<2>(), IC<0>(), pc, gc, s, bo, bn);
+        phase_B(IC<1>(), IC<0>(), ph_, gh, s, bo, bn);
       }
-      iter_end(IC<1>(), k);
+      odd = !odd;
+      iter_end(IC<1>(), i);
     }
   } else {
     // ============================ phase warps ============================
@@ -732,26 +739,28 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     const int pnj = min(z1, P.out_hi ? L.nz - 1 : L.nz) - pjlo;
     const int pnjs0 = (gx_ >= xs && gy_ >= ys) ? pnj : 0, pnjs1 = (gx_ >= xs && gy_ + 2 >= ys) ? pnj : 0;
     T *pph = P.out.f[F_PHI] + o00 + (long long)(kst - 1) * L.plane;   // phi of the first pair, plane k-1
+    const int pju = kst - 1 - pjlo;          // (plane k-1) - pjlo = i + pju
+    int bo = (kst & 1) * BUF;
     for (int i = 0; i < NI; ++i) {
-      const int k = kst + i;
-      const int bo = (k & 1) * BUF, bn = BUF - bo;
-      if (has_group(k)) mbar_wait(&bars[s], mph);
-      if (k <= z1) {
-        if (k - 1 >= z0) phase_D(IC<0>(), g0.oZ, g0.oT, s, bn, eoff, emask, esign);   // (rows r + 2: the halo-row warp)
-        const V f0 = phase_B(IC<0>(), IC<0>(), p0, g0, k, s, bo, bn);
-        const V f1 = phase_B(IC<0>(), IC<2>(), p1, g0, k, s, bo, bn);
+      const int bn = BUF - bo;
+      if (i <= IZ1) {
+        mbar_wait(&bars[s], mph);
+        if (i >= I0 + 1) phase_D(IC<0>(), g0.oZ, g0.oT, s, bn, eoff, emask, esign);   // (rows r + 2: the halo-row warp)
+        const V f0 = phase_B(IC<0>(), IC<0>(), p0, g0, s, bo, bn);
+        const V f1 = phase_B(IC<0>(), IC<2>(), p1, g0, s, bo, bn);
         // a9: phi'(k-1) of the two pairs
-        const bool in0 = (unsigned)(k - 1 - pjlo) < (unsigned)pnjs0, in1 = (unsigned)(k - 1 - pjlo) < (unsigned)pnjs1;
+        const bool in0 = (unsigned)(i + pju) < (unsigned)pnjs0, in1 = (unsigned)(i + pju) < (unsigned)pnjs1;
         stg_pair_if(in0, pph, f0);
         stg_pair_if(in1, pph + 2 * L.px, f1);
         if (img0 || img1 || SLAB) {
           V o[NF_MAX];
-          if (in0) { o[F_PHI] = f0; store_rare<T, FM_PHI, SLAB>(P, o, k - 1, gx_, gy_, img0); }
-          if (in1) { o[F_PHI] = f1; store_rare<T, FM_PHI, SLAB>(P, o, k - 1, gx_, gy_ + 2, img1); }
+          if (in0) { o[F_PHI] = f0; store_rare<T, FM_PHI, SLAB>(P, o, kst + i - 1, gx_, gy_, img0); }
+          if (in1) { o[F_PHI] = f1; store_rare<T, FM_PHI, SLAB>(P, o, kst + i - 1, gx_, gy_ + 2, img1); }
         }
       }
       pph += L.plane;
-      iter_end(IC<0>(), k);
+      bo = bn;
+      iter_end(IC<0>(), i);
     }
   }
 }
