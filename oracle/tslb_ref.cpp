@@ -22,9 +22,13 @@
  * is silent on how the force enters; A18 is pinned by the published scheme's moment conditions,
  * momentum balance, closed-form forced flows and a numpy restatement (tests/test_oracle_forcing.py).
  *
- * Parity pins: tests/test_oracle_*.py.  Unpinned by the paper: the inflow/outflow details
- * (A10, A11) -- "parity unpinned" for those two planes; they are checked for boundedness,
- * inlet mass flux and oracle<->GPU agreement only.
+ * Parity pins: tests/test_oracle_*.py (one named pin per function: DESIGN.md section 2).  The inflow /
+ * outflow READING (A10, A11: which values are imposed on the two planes, and from which time level) is
+ * not fixed by the paper; what boundary_planes() does with that reading is pinned: the populations it
+ * rebuilds are eq. 9 (test_jet_boundary_populations_are_eq9), the interior mass changes by exactly what
+ * they carry in and out and the inlet flux is sum_nozzle rho_B U (1 + p xi)
+ * (test_jet_mass_balance_from_boundary_populations), and under A18 the two planes carry no force
+ * (test_guo_jet_momentum_balance_with_unforced_boundary_planes).
  */
 #include "tslb_ref.h"
 
