@@ -103,7 +103,7 @@ Validated validate(const tslb_params *p) {
   v.esize = p->precision == TSLB_F32 ? 4 : 8;
   v.nfields = p->two_component ? 11 : 10;
   v.L = make_layout(p->nx, p->ny, p->nz, v.slab ? GZ : 0);
-  const bool tiled_ok = tiled_supported(p->precision, p->nx, p->ny, p->nz);
+  const bool tiled_ok = tiled_supported(p->precision, p->two_component != 0, p->nx, p->ny, p->nz);
   if (p->kernel == TSLB_KERNEL_TILED && !tiled_ok)
     return fail("TSLB_KERNEL_TILED needs nx >= 32, ny >= 8 and nx a multiple of 4 (fp32) or 2 (fp64)");
   v.kernel = (p->kernel == TSLB_KERNEL_GENERIC || !tiled_ok || guo) ? TSLB_KERNEL_GENERIC : TSLB_KERNEL_TILED;

@@ -75,7 +75,13 @@ template <typename T, int TX_, int TY_, bool TWO>
 struct TileCfg {
   static constexpr int TX = TX_, TY = TY_;
   static constexpr int LX = TX / 2;        // threads per row (two nodes each)
-  static_assert(LX == 16 && TY % 4 == 0, "a warp owns two rows of 16 node pairs; a phase warp four rows");
+  // UNI (fp64, two components): ONE copy of the phase code.  Every phase thread owns one node pair, and the
+  // pairs of the two halo rows are owned by a phase warp of their own that runs the same code with its
+  // stores switched off, so that the code the SM's warps loop over fits the 32 KB instruction cache (the
+  // fp64 code of the fp32 arrangement does not: DESIGN.md 6.4).  The warps then fall into register classes
+  // by warpgroup (setmaxnreg): warps 0-3 flow + halo-row x-pass, 4-7 phase, 8 halo columns.
+  static constexpr bool UNI = TWO && sizeof(T) == 8;
+  static_assert(LX == 16 && TY % (UNI ? 2 : 4) == 0, "a warp owns two rows of 16 node pairs; a phase warp four rows (UNI: two)");
   // left/right staged halo columns.  2 are needed; the TMA box row must be a multiple of 32 bytes
   // (16-byte-odd rows raised "illegal instruction" on B200), so fp32 stages 4.
   static constexpr int HL = sizeof(T) == 4 ? 4 : 2;
@@ -86,9 +92,12 @@ struct TileCfg {
   // warp roles: NWF flow warps (two tile rows each), the halo-row warp, the halo-column warp, and (two-
   // component) NWP phase warps that own the phase field of four tile rows each
   static constexpr int NWF = TY / 2;
-  static constexpr int NWP = TWO ? TY / 4 : 0;
-  static constexpr int W_HALO = NWF, W_COL = NWF + 1, W_PH0 = NWF + 2;
-  static constexpr int NTHREADS = 32 * (NWF + 2 + NWP);
+  static constexpr int NWP = TWO ? (UNI ? TY / 2 + 1 : TY / 4) : 0;
+  static constexpr int W_HALO = NWF, W_COL = UNI ? NWF + 1 + NWP : NWF + 1, W_PH0 = UNI ? NWF + 1 : NWF + 2;
+  static_assert(!UNI || (NWF + 1 == 4 && NWP == 4), "UNI: the flow warps and the phase warps are one warpgroup each");
+  // (UNI: the halo-column warp's warpgroup is filled up with three idle warps -- setmaxnreg is a warpgroup
+  // instruction, and the register pool of the CTA is what its warps were launched with)
+  static constexpr int NTHREADS = UNI ? 384 : 32 * (NWF + 2 + NWP);
   static constexpr int NXPASS = 32 * (NWF + 1);          // threads that take part in the x-pass / y-push
   static_assert(2 * RY < 32, "the halo-column warp has one lane per halo-column node and a spare lane");
   static constexpr int NYP = 9;            // y-push fields per direction: (c,p)
@@ -114,7 +123,8 @@ struct TileCfg {
   static constexpr int B_FQ = B_GQ + (TWO ? 2 * GQE : 0);        // [2]  (phi + q_x).y, (phi - q_x).x per pair
   static constexpr int B_KF = B_FQ + (TWO ? 2 * FQE : 0);        // [3]  F = sigma kappa grad(phi), phase -> flow
   static constexpr int B_PH = B_KF + (TWO ? 3 * TLE : 0);        // [1]  own phi, private to the owning phase thread
-  static constexpr int BUF = (B_PH + (TWO ? TLE : 0) + 3) / 4 * 4;   // elements per half
+  static constexpr int PHE = UNI ? GQE : TLE;                    //      (UNI: of the halo-row pairs too)
+  static constexpr int BUF = (B_PH + (TWO ? PHE : 0) + 3) / 4 * 4;   // elements per half
   static_assert(ZCE % 2 == 0 && ZLE % 2 == 0 && GQE % 2 == 0 && FQE % 2 == 0, "pair alignment");
   // y-push field: TY sending rows, and one more row that holds the x-pass terms of a halo column for the
   // lanes at the tile edge ([2 plane parities][RY]; a+ of column x0-1 in the a+ fields, a- of column
@@ -144,11 +154,29 @@ struct TiledMaps {
 };
 
 // Reciprocal and square root.  fp32: the branch-free MUFU approximations (<= 2 ulp, far inside the
-// 1e-5 parity gate; rho' ~ 1 and |G| + eps >= 1e-12 are normal numbers); fp64: IEEE.
+// 1e-5 parity gate; rho' ~ 1 and |G| + eps >= 1e-12 are normal numbers).  fp64: the 20-bit MUFU seed and
+// two Newton steps (+ a residual step for the root), branch-free: the compiler's IEEE sequences carry an
+// out-of-line special-case path that sqrt(0) -- every node away from the interface -- takes, and the
+// code has to stay inside the instruction cache.  Within 1 ulp of the IEEE result; a root of less than
+// 1e-140 (its square is flushed by the seed) is returned as 0, which moves n = G/(|G| + 1e-12) by < 1e-128.
 __device__ __forceinline__ float rcp1(float s) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(s)); return r; }
-__device__ __forceinline__ double rcp1(double s) { return 1.0 / s; }
+__device__ __forceinline__ double rcp1(double s) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(s));
+  r = fma(r, fma(-s, r, 1.0), r);
+  return fma(r, fma(-s, r, 1.0), r);
+}
 __device__ __forceinline__ float sqrt1(float s) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(s)); return r; }
-__device__ __forceinline__ double sqrt1(double s) { return sqrt(s); }
+__device__ __forceinline__ double sqrt1(double s) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(s));
+  double g = s * y, h = 0.5 * y, e = fma(-g, h, 0.5);
+  g = fma(g, e, g); h = fma(h, e, h);
+  e = fma(-g, h, 0.5);
+  g = fma(g, e, g); h = fma(h, e, h);
+  g = fma(fma(-g, g, s), h, g);
+  return s < 1e-280 ? 0.0 : g;
+}
 template <typename T> __device__ __forceinline__ Pair<T> prcp(Pair<T> a) { return Pair<T>(rcp1(a.x), rcp1(a.y)); }
 
 // predicated shared-memory pair store (kept as ONE predicated instruction: a branch around a store
@@ -315,6 +343,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   constexpr int LX = C::LX, HL = C::HL, RX = C::RX, RY = C::RY, S = C::S, ZW = C::ZW, FQW = C::FQW;
   constexpr int ZCE = C::ZCE, ZLE = C::ZLE, GQE = C::GQE, FQE = C::FQE, TLE = C::TLE, YPF = C::YPF, BUF = C::BUF;
   constexpr int MF = RY * RX;                           // elements per moment field in a stage
+  constexpr bool UNI = C::UNI;
   extern __shared__ __align__(128) unsigned char smem[];
   uint64_t *bars = reinterpret_cast<uint64_t *>(smem + C::OFF_BAR);
   auto mom_at = [&](int slot) { return reinterpret_cast<T *>(smem + C::OFF_MOM + slot * C::MOM_STAGE); };
@@ -330,11 +359,15 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   const bool flow = wid < C::NWF;                         // owns the flow of two tile rows
   const bool halow = wid == C::W_HALO;
   const bool colw = wid == C::W_COL;
+  const bool phalo = UNI && wid == C::W_PH0 + C::NWP - 1;   // UNI: the phase warp of the two halo rows
+  const bool dwarp = UNI && wid > C::W_COL;                 // UNI: the three warps that run D (tile rows like the flow warps)
   const int lx = lane & (LX - 1), hi = lane >> 4;
   // region row (y = y0 - 1 + r) of the thread's (first) node pair and staged column of its first node
   const int r = flow ? 2 * wid + 1 + hi
                      : (halow ? (hi ? 0 : RY - 1)
-                              : (colw ? (lane < RY ? lane : (lane < 2 * RY ? lane - RY : 0)) : 4 * (wid - C::W_PH0) + 1 + hi));
+                              : (colw ? (lane < RY ? lane : (lane < 2 * RY ? lane - RY : 0))
+                                      : (UNI ? (phalo ? (hi ? 0 : RY - 1) : 2 * (wid - (dwarp ? C::W_COL + 1 : C::W_PH0)) + 1 + hi)
+                                             : 4 * (wid - C::W_PH0) + 1 + hi)));
   const int cside = lane >= RY;                           // halo-column warp: 0 left, 1 right
   const int c0 = colw ? (cside ? HL + TX : HL - 2) : HL + 2 * lx;
   int oM = r * RX + c0;                                   // offset of the pair in a staged region plane
@@ -444,7 +477,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     V ph;                                                               // own phi(k)
     if (ROLE == 0) {
       // tile pairs keep their own phi(k), phi(k+1) in a private two-slot ring (slot = plane parity)
-      T *pr = s_buf + bo + C::B_PH + g.oT;
+      T *pr = s_buf + bo + C::B_PH + (UNI ? g.oG : g.oT);
       ph = lds_pair(pr);
       sts_pair(pr, cb);
     } else {
@@ -468,7 +501,8 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
       const V qz = pfma(bq, st.nB[2], a4 * lds_pair(mo + F_UZ * MF));
       // grad(phi) of plane k+1 for the kick two iterations on -> ring slot s
       T *gr_ = s_gr + s * 3 * TLE + g.oT;
-      sts_pair(gr_, gx); sts_pair(gr_ + TLE, gy); sts_pair(gr_ + 2 * TLE, gz);
+      if (UNI) { sts_pair_if(!phalo, gr_, gx); sts_pair_if(!phalo, gr_ + TLE, gy); sts_pair_if(!phalo, gr_ + 2 * TLE, gz); }
+      else { sts_pair(gr_, gx); sts_pair(gr_ + TLE, gy); sts_pair(gr_ + 2 * TLE, gz); }
       // phi'(k-1) = phi/4 + (in-plane arrivals of plane k-1 + up(k-2) + down(k)) / 8
       const T *fr = s_buf + bn + C::B_FQ + g.oF;
       const T *gr = s_buf + bn + C::B_GQ + g.oG;
@@ -581,6 +615,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
 
   if (flow || halow) {
     // ============================ flow warps and the halo-row warp ============================
+    if (UNI) asm volatile("setmaxnreg.inc.sync.aligned.u32 248;");
     V accA[10], accB[10];     // Hermite moments being accumulated for planes k and k+1
     V ubx(T(0)), uby(T(0)), ubz(T(0)), rinv(T(1));   // u_b and 1/rho' of the plane completed last
 #pragma unroll
@@ -606,7 +641,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
       V A0[9];                               // own y-push term a0 per (c,p)
       if (src) xpass(odd, s, A0);
       xpass_barrier();
-      if (TWO && halow && i <= IZ1 && i >= I0 + 1) {
+      if (TWO && !UNI && halow && i <= IZ1 && i >= I0 + 1) {
         phase_D(IC<0>(), dZ, dT, s, BUF - bo, deoff, demask, design);
         phase_D(IC<4>(), dZ, dT, s, BUF - bo, deoff, demask, design);
       }
@@ -677,8 +712,23 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
       odd = !odd;
       iter_end(IC<0>(), i);
     }
-  } else if (colw) {
+  } else if (colw || dwarp) {
     // ============================ halo-column warp ============================
+    if (UNI) asm volatile("setmaxnreg.dec.sync.aligned.u32 112;");
+    if (dwarp) {
+      // UNI: the other three warps of its warpgroup run D (it carries no state from plane to plane)
+      const int oZ = r * ZW + 2 + 2 * lx;
+      const int eoff = (lx == 0 ? C::B_ZL : (lx == LX - 1 ? C::B_ZL + RY : C::B_ZZ)) + 2 + r;
+      const V emask(lx == 0 ? T(1) : T(0), lx == LX - 1 ? T(1) : T(0));
+      const T esign = lx == 0 ? T(-0.5) : T(0.5);
+      int bo = (kst & 1) * BUF;
+      for (int i = 0; i < NI; ++i) {
+        const int bn = BUF - bo;
+        if (i <= IZ1 && i >= I0 + 1) phase_D(IC<0>(), oZ, oT, s, bn, eoff, emask, esign);
+        bo = bn;
+        iter_end(IC<0>(), i);
+      }
+    } else {
     // node pairs: lanes 0 .. 2 RY - 1 own the two halo columns; every lane owns a pair of the halo rows
     PhaseState<T> pc, ph_;
     pc.clear(); ph_.clear();
@@ -717,14 +767,16 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
       }
       if (TWO && i <= IZ1) {
         if (lane < 2 * RY) phase_B(IC<2>(), IC<0>(), pc, gc, s, bo, bn);
-        phase_B(IC<1>(), IC<0>(), ph_, gh, s, bo, bn);
+        if (!UNI) phase_B(IC<1>(), IC<0>(), ph_, gh, s, bo, bn);   // (UNI: a phase warp owns the halo rows)
       }
       odd = !odd;
       iter_end(IC<1>(), i);
     }
+    }
   } else {
     // ============================ phase warps ============================
-    PhaseState<T> p0, p1;     // two node pairs: rows r and r + 2
+    if (UNI) asm volatile("setmaxnreg.dec.sync.aligned.u32 136;");
+    PhaseState<T> p0, p1;     // two node pairs: rows r and r + 2 (UNI: one)
     p0.clear(); p1.clear();
     const int oZ = r * ZW + 2 + 2 * lx, oF = r * FQW + 1 + lx, oG = r * TX + 2 * lx;
     const PairGeom g0 = {r * RX, c0, c0 - 1, c0 + 2, oZ, oF, oG, oT};
@@ -737,7 +789,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     // planes; nothing when the node belongs to the neighbouring (shifted-back) tile
     const int pjlo = max(z0, P.jet_lo ? 1 : 0);
     const int pnj = min(z1, P.out_hi ? L.nz - 1 : L.nz) - pjlo;
-    const int pnjs0 = (gx_ >= xs && gy_ >= ys) ? pnj : 0, pnjs1 = (gx_ >= xs && gy_ + 2 >= ys) ? pnj : 0;
+    const int pnjs0 = (!phalo && gx_ >= xs && gy_ >= ys) ? pnj : 0, pnjs1 = (gx_ >= xs && gy_ + 2 >= ys) ? pnj : 0;
     T *pph = P.out.f[F_PHI] + o00 + (long long)(kst - 1) * L.plane;   // phi of the first pair, plane k-1
     const int pju = kst - 1 - pjlo;          // (plane k-1) - pjlo = i + pju
     int bo = (kst & 1) * BUF;
@@ -745,6 +797,17 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
       const int bn = BUF - bo;
       if (i <= IZ1) {
         mbar_wait(&bars[s], mph);
+        if (UNI) {
+          // one pair per thread; the warp of the halo rows runs the same code and stores nothing
+          // (D: the three spare warps of the halo-column warp's warpgroup)
+          const V f0 = phase_B(IC<0>(), IC<0>(), p0, g0, s, bo, bn);
+          const bool in0 = (unsigned)(i + pju) < (unsigned)pnjs0;
+          stg_pair_if(in0, pph, f0);
+          if ((img0 || SLAB) && in0) {
+            V o[NF_MAX];
+            o[F_PHI] = f0; store_rare<T, FM_PHI, SLAB>(P, o, kst + i - 1, gx_, gy_, img0);
+          }
+        } else {
         if (i >= I0 + 1) phase_D(IC<0>(), g0.oZ, g0.oT, s, bn, eoff, emask, esign);   // (rows r + 2: the halo-row warp)
         const V f0 = phase_B(IC<0>(), IC<0>(), p0, g0, s, bo, bn);
         const V f1 = phase_B(IC<0>(), IC<2>(), p1, g0, s, bo, bn);
@@ -756,6 +819,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
           V o[NF_MAX];
           if (in0) { o[F_PHI] = f0; store_rare<T, FM_PHI, SLAB>(P, o, kst + i - 1, gx_, gy_, img0); }
           if (in1) { o[F_PHI] = f1; store_rare<T, FM_PHI, SLAB>(P, o, kst + i - 1, gx_, gy_ + 2, img1); }
+        }
         }
       }
       pph += L.plane;
@@ -780,18 +844,18 @@ struct TiledPlan {
   bool two = false;
 };
 
-// tile shapes: 32x8 in both precisions (fp32: ~103 KB of shared memory -> two CTAs per SM, whose
-// barrier phases interleave; measured 30.2 vs 27.6 GLUPS for 64x8 on C5)
-constexpr int TILE_TX = 32, TILE_TY = 8;
-inline void tiled_tile(int precision, int &tx, int &ty) {
-  (void)precision;
+// tile shapes: 32x8 (fp32: ~103 KB of shared memory -> two CTAs per SM, whose barrier phases interleave;
+// measured 30.2 vs 27.6 GLUPS for 64x8 on C5); 32x6 for the two-component fp64 build (TileCfg::UNI: three
+// flow warps + the halo-row warp are one warpgroup, three phase warps + the halo rows' phase warp another)
+constexpr int TILE_TX = 32, TILE_TY = 8, TILE_TY_UNI = 6;
+inline void tiled_tile(int precision, bool two, int &tx, int &ty) {
   tx = TILE_TX;
-  ty = TILE_TY;
+  ty = precision == TSLB_F64 && two ? TILE_TY_UNI : TILE_TY;
 }
 
-inline bool tiled_supported(int precision, int nx, int ny, int nz) {
+inline bool tiled_supported(int precision, bool two, int nx, int ny, int nz) {
   int tx, ty;
-  tiled_tile(precision, tx, ty);
+  tiled_tile(precision, two, tx, ty);
   // rows of the padded arrays must be multiples of 16 bytes for TMA (px = nx + 16)
   return nx % (precision == TSLB_F32 ? 4 : 2) == 0 && nz >= 1 && nx >= tx && ny >= ty;
 }
@@ -808,7 +872,7 @@ inline bool tiled_plan_create(TiledPlan &pl, int precision, const Layout &L, voi
   }
   pl.precision = precision;
   pl.two = nfields == 11;
-  tiled_tile(precision, pl.tx, pl.ty);
+  tiled_tile(precision, pl.two, pl.tx, pl.ty);
   const size_t es = precision == TSLB_F32 ? 4 : 8;
   const CUtensorMapDataType dt = precision == TSLB_F32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64;
   const int RX = pl.tx + 2 * (es == 4 ? 4 : 2), RY = pl.ty + 2, RYP = pl.ty + 4;
@@ -877,13 +941,14 @@ __global__ void tiled_boundary_kernel(const __grid_constant__ StepParams<T> P, i
   for (int k = 0; k < nf; ++k) P.out.f[k][i0] = o[k];
 }
 
-template <typename T, int TX, int TY>
-cudaError_t launch_tiled_t(TiledPlan &pl, const StepParams<T> &P, int src, int order, bool two, cudaStream_t st) {
+template <typename T, int TX, int TY, bool TWOC>
+cudaError_t launch_tiled_t(TiledPlan &pl, const StepParams<T> &P, int src, int order, cudaStream_t st) {
+  constexpr bool two = TWOC;
   const bool slab = P.halo_lo || P.halo_hi;
   const TiledMaps &M = pl.maps[src];
   dim3 grid(M.ntx * M.nty, (P.L.nz + M.zc - 1) / M.zc);
   cudaError_t e = cudaSuccess;
-#define TSLB_LAUNCH(ORD, TWOC, SL)                                                                      \
+#define TSLB_LAUNCH(ORD, SL)                                                                            \
   do {                                                                                                \
     using Cf = TileCfg<T, TX, TY, TWOC>;                                                              \
     auto kern = tiled_step_kernel<T, TX, TY, ORD, TWOC, SL>;                                          \
@@ -895,13 +960,8 @@ cudaError_t launch_tiled_t(TiledPlan &pl, const StepParams<T> &P, int src, int o
     }                                                                                                 \
     kern<<<grid, Cf::NTHREADS, Cf::SMEM_BYTES, st>>>(P, M);                                           \
   } while (0)
-  if (slab) {
-    if (two) { if (order >= 3) TSLB_LAUNCH(3, true, true); else TSLB_LAUNCH(2, true, true); }
-    else     { if (order >= 3) TSLB_LAUNCH(3, false, true); else TSLB_LAUNCH(2, false, true); }
-  } else {
-    if (two) { if (order >= 3) TSLB_LAUNCH(3, true, false); else TSLB_LAUNCH(2, true, false); }
-    else     { if (order >= 3) TSLB_LAUNCH(3, false, false); else TSLB_LAUNCH(2, false, false); }
-  }
+  if (slab) { if (order >= 3) TSLB_LAUNCH(3, true); else TSLB_LAUNCH(2, true); }
+  else      { if (order >= 3) TSLB_LAUNCH(3, false); else TSLB_LAUNCH(2, false); }
 #undef TSLB_LAUNCH
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;
@@ -917,11 +977,13 @@ template <typename T>
 cudaError_t launch_tiled(TiledPlan &pl, const StepParams<T> &P, int src, int order, bool two, cudaStream_t st);
 template <>
 inline cudaError_t launch_tiled<float>(TiledPlan &pl, const StepParams<float> &P, int src, int order, bool two, cudaStream_t st) {
-  return launch_tiled_t<float, TILE_TX, TILE_TY>(pl, P, src, order, two, st);
+  return two ? launch_tiled_t<float, TILE_TX, TILE_TY, true>(pl, P, src, order, st)
+             : launch_tiled_t<float, TILE_TX, TILE_TY, false>(pl, P, src, order, st);
 }
 template <>
 inline cudaError_t launch_tiled<double>(TiledPlan &pl, const StepParams<double> &P, int src, int order, bool two, cudaStream_t st) {
-  return launch_tiled_t<double, TILE_TX, TILE_TY>(pl, P, src, order, two, st);
+  return two ? launch_tiled_t<double, TILE_TX, TILE_TY_UNI, true>(pl, P, src, order, st)
+             : launch_tiled_t<double, TILE_TX, TILE_TY, false>(pl, P, src, order, st);
 }
 
 }  // namespace tslb
