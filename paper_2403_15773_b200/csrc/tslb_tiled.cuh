@@ -75,11 +75,13 @@ template <typename T, int TX_, int TY_, bool TWO>
 struct TileCfg {
   static constexpr int TX = TX_, TY = TY_;
   static constexpr int LX = TX / 2;        // threads per row (two nodes each)
-  // UNI (fp64, two components): ONE copy of the phase code.  Every phase thread owns one node pair, and the
-  // pairs of the two halo rows are owned by a phase warp of their own that runs the same code with its
-  // stores switched off, so that the code the SM's warps loop over fits the 32 KB instruction cache (the
-  // fp64 code of the fp32 arrangement does not: DESIGN.md 6.4).  The warps then fall into register classes
-  // by warpgroup (setmaxnreg): warps 0-3 flow + halo-row x-pass, 4-7 phase, 8 halo columns.
+  // UNI (fp64, two components): ONE copy of the phase code -- every phase thread owns one
+  // node pair, and the pairs of the two halo rows are owned by a phase warp of their own that runs the same
+  // code with its stores switched off -- so that the code the SM's warps loop over fits the 32 KB instruction
+  // cache; and the flow work of a plane is split between the warps that form the x-pass / y-push terms (A)
+  // and the warps that pull them one iteration later, push along z, finish and store the plane (C, D), so
+  // that no warp carries more than ~500 instructions per plane.  Register classes by warpgroup (setmaxnreg):
+  // warps 0-3 A (three for the tile rows, one for the halo rows), 4-6 C + D and 7 the halo columns, 8-11 phase.
   static constexpr bool UNI = TWO && sizeof(T) == 8;
   static_assert(LX == 16 && TY % (UNI ? 2 : 4) == 0, "a warp owns two rows of 16 node pairs; a phase warp four rows (UNI: two)");
   // left/right staged halo columns.  2 are needed; the TMA box row must be a multiple of 32 bytes
@@ -93,10 +95,10 @@ struct TileCfg {
   // component) NWP phase warps that own the phase field of four tile rows each
   static constexpr int NWF = TY / 2;
   static constexpr int NWP = TWO ? (UNI ? TY / 2 + 1 : TY / 4) : 0;
-  static constexpr int W_HALO = NWF, W_COL = UNI ? NWF + 1 + NWP : NWF + 1, W_PH0 = UNI ? NWF + 1 : NWF + 2;
-  static_assert(!UNI || (NWF + 1 == 4 && NWP == 4), "UNI: the flow warps and the phase warps are one warpgroup each");
-  // (UNI: the halo-column warp's warpgroup is filled up with three idle warps -- setmaxnreg is a warpgroup
-  // instruction, and the register pool of the CTA is what its warps were launched with)
+  static constexpr int W_HALO = NWF, W_C0 = NWF + 1;          // (W_C0: UNI, first of the NWF C warps)
+  static constexpr int W_COL = UNI ? W_C0 + NWF : NWF + 1, W_PH0 = UNI ? W_COL + 1 : NWF + 2;
+  static_assert(!UNI || (NWF + 1 == 4 && NWP == 4), "UNI: A warps, C warps + halo-column warp, phase warps: a warpgroup each");
+  // (setmaxnreg is a warpgroup instruction, and the register pool of the CTA is what its warps were launched with)
   static constexpr int NTHREADS = UNI ? 384 : 32 * (NWF + 2 + NWP);
   static constexpr int NXPASS = 32 * (NWF + 1);          // threads that take part in the x-pass / y-push
   static_assert(2 * RY < 32, "the halo-column warp has one lane per halo-column node and a spare lane");
@@ -122,7 +124,7 @@ struct TileCfg {
   static constexpr int B_GQ = B_ZZ + (TWO ? 3 * ZLE : 0);        // [2]  phi + q_y, phi - q_y
   static constexpr int B_FQ = B_GQ + (TWO ? 2 * GQE : 0);        // [2]  (phi + q_x).y, (phi - q_x).x per pair
   static constexpr int B_KF = B_FQ + (TWO ? 2 * FQE : 0);        // [3]  F = sigma kappa grad(phi), phase -> flow
-  static constexpr int B_PH = B_KF + (TWO ? 3 * TLE : 0);        // [1]  own phi, private to the owning phase thread
+  static constexpr int B_PH = B_KF + (TWO && !UNI ? 3 * TLE : 0);   // [1]  own phi, private to the owning phase thread
   static constexpr int PHE = UNI ? GQE : TLE;                    //      (UNI: of the halo-row pairs too)
   static constexpr int BUF = (B_PH + (TWO ? PHE : 0) + 3) / 4 * 4;   // elements per half
   static_assert(ZCE % 2 == 0 && ZLE % 2 == 0 && GQE % 2 == 0 && FQE % 2 == 0, "pair alignment");
@@ -139,10 +141,15 @@ struct TileCfg {
   // grad(phi) of the tile nodes, written by the phase thread that owns the pair and read two iterations
   // later by whoever forms F: a ring of three slots (slot = TMA ring slot of the writing iteration)
   static constexpr size_t OFF_GR = OFF_BUF + (size_t)2 * BUF * sizeof(T);   // [3][3][TLE]
-  static constexpr size_t OFF_AP = OFF_GR + (TWO ? (size_t)9 * TLE * sizeof(T) : 0);   // [9]
-  static constexpr size_t OFF_AM = OFF_AP + (size_t)NYP * YPF * sizeof(T);  // [9]
-  static constexpr size_t OFF_BAR = OFF_AM + (size_t)NYP * YPF * sizeof(T);
+  // (UNI: the y-push fields and the rows' own terms a0 cross an iteration -- A writes, C reads one iteration
+  // later -- and exist twice, by plane parity)
+  static constexpr int NCOPY = UNI ? 2 : 1;
+  static constexpr size_t OFF_AP = OFF_GR + (TWO ? (size_t)9 * TLE * sizeof(T) : 0);   // [NCOPY][9][YPF]
+  static constexpr size_t OFF_AM = OFF_AP + (size_t)NCOPY * NYP * YPF * sizeof(T);     // [NCOPY][9][YPF]
+  static constexpr size_t OFF_A0 = OFF_AM + (size_t)NCOPY * NYP * YPF * sizeof(T);     // UNI: [2][9][TLE]
+  static constexpr size_t OFF_BAR = OFF_A0 + (UNI ? (size_t)2 * NYP * TLE * sizeof(T) : 0);
   static constexpr size_t SMEM_BYTES = OFF_BAR + 64;
+  static_assert(SMEM_BYTES <= 227 * 1024, "shared memory of one CTA");
   static constexpr int CTAS_PER_SM = SMEM_BYTES <= 113 * 1024 ? 2 : 1;
 };
 
@@ -350,8 +357,9 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   auto phi_at = [&](int slot) { return reinterpret_cast<T *>(smem + C::OFF_PHI + slot * C::PHI_STAGE); };
   T *s_buf = reinterpret_cast<T *>(smem + C::OFF_BUF);     // [2][BUF]
   T *s_gr = reinterpret_cast<T *>(smem + C::OFF_GR);       // [3][3][TLE]
-  T *s_ap = reinterpret_cast<T *>(smem + C::OFF_AP);       // [9][YPF]
+  T *s_ap = reinterpret_cast<T *>(smem + C::OFF_AP);       // [9][YPF]  (UNI: [2][9][YPF], by plane parity)
   T *s_am = reinterpret_cast<T *>(smem + C::OFF_AM);
+  T *s_a0 = reinterpret_cast<T *>(smem + C::OFF_A0);       // UNI: [2][9][TLE]
 
   const Layout &L = P.L;
   const int t = threadIdx.x;
@@ -360,13 +368,13 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   const bool halow = wid == C::W_HALO;
   const bool colw = wid == C::W_COL;
   const bool phalo = UNI && wid == C::W_PH0 + C::NWP - 1;   // UNI: the phase warp of the two halo rows
-  const bool dwarp = UNI && wid > C::W_COL;                 // UNI: the three warps that run D (tile rows like the flow warps)
+  const bool cwarp = UNI && wid >= C::W_C0 && wid < C::W_COL;   // UNI: the warps that run C and D (tile rows like the A warps)
   const int lx = lane & (LX - 1), hi = lane >> 4;
   // region row (y = y0 - 1 + r) of the thread's (first) node pair and staged column of its first node
   const int r = flow ? 2 * wid + 1 + hi
                      : (halow ? (hi ? 0 : RY - 1)
                               : (colw ? (lane < RY ? lane : (lane < 2 * RY ? lane - RY : 0))
-                                      : (UNI ? (phalo ? (hi ? 0 : RY - 1) : 2 * (wid - (dwarp ? C::W_COL + 1 : C::W_PH0)) + 1 + hi)
+                                      : (UNI ? (phalo ? (hi ? 0 : RY - 1) : 2 * (wid - (cwarp ? C::W_C0 : C::W_PH0)) + 1 + hi)
                                              : 4 * (wid - C::W_PH0) + 1 + hi)));
   const int cside = lane >= RY;                           // halo-column warp: 0 left, 1 right
   const int c0 = colw ? (cside ? HL + TX : HL - 2) : HL + 2 * lx;
@@ -520,7 +528,8 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   // warp, which has time to spare): kappa(k-1) = -(S_y ax + D_y bx + S_y cx) from the x-combined
   // z-combinations of n written in iteration k-1, plus the share of the halo column for the lanes at the tile edge (every other lane reads zeros
   // through the same per-lane pointer: no divergence); F(k-1) = sigma kappa grad(phi)(k-1) -> flow warps.
-  auto phase_D = [&](auto drc, int oZ0, int oT0, int s, int bn, int eoff, V emask, T esign) {
+  // (UNI: the C warp that runs D keeps F in registers, Fr, for its own kick one iteration later)
+  auto phase_D = [&](auto drc, int oZ0, int oT0, int s, int bn, int eoff, V emask, T esign, V *Fr) {
     constexpr int DR = decltype(drc)::value;
     const PairGeom g = {0, 0, 0, 0, oZ0 + DR * ZW, 0, 0, oT0 + DR * TX};
     const T *zr = s_buf + bn + C::B_ZC + g.oZ;
@@ -535,10 +544,14 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     kap = pfma(V(corr), emask, kap);
     const V sc = kap * (-P.sigma);                                       // F = sigma kappa G, kappa = -kap
     const T *gr_ = s_gr + (s == S - 1 ? 0 : s + 1) * 3 * TLE + g.oT;      // G(k-1): written two iterations ago
-    T *kf = s_buf + bn + C::B_KF + g.oT;
-    sts_pair(kf, lds_pair(gr_) * sc);
-    sts_pair(kf + TLE, lds_pair(gr_ + TLE) * sc);
-    sts_pair(kf + 2 * TLE, lds_pair(gr_ + 2 * TLE) * sc);
+    if (UNI) {
+      Fr[0] = lds_pair(gr_) * sc; Fr[1] = lds_pair(gr_ + TLE) * sc; Fr[2] = lds_pair(gr_ + 2 * TLE) * sc;
+    } else {
+      T *kf = s_buf + bn + C::B_KF + g.oT;
+      sts_pair(kf, lds_pair(gr_) * sc);
+      sts_pair(kf + TLE, lds_pair(gr_ + TLE) * sc);
+      sts_pair(kf + 2 * TLE, lds_pair(gr_ + 2 * TLE) * sc);
+    }
   };
 
   // ring slot of this iteration's group (group kfirst sits in slot 0) and its mbarrier phase parity
@@ -569,9 +582,10 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   const int hpar = (lx == 0 ? 1 : 0) | (lx == LX - 1 ? 2 : 0);
   auto xpass = [&](bool odd, int s, V (&A0)[9]) {      // odd: parity of the plane
     const int oAM = oAP - 2 * TX;
-    T *const xp = s_ap + oXP, *const xm = s_am + oXM;
-    const int hoff = odd ? RY : 0;
-    const T *pl = s_ap + oPL + ((hpar & 1) ? hoff : 0), *pr = s_am + oPR + ((hpar & 2) ? hoff : 0);
+    const int yoff = UNI && odd ? C::NYP * YPF : 0;    // UNI: the copy of the y-push fields of this parity
+    T *const xp = s_ap + oXP + yoff, *const xm = s_am + oXM + yoff;
+    const int hoff = odd ? RY : 0;                     // (the halo-column terms: always in copy 0)
+    const T *pl = s_ap + oPL + ((hpar & 1) ? hoff : yoff), *pr = s_am + oPR + ((hpar & 2) ? hoff : yoff);
     V Xg[8][3];   // [group][p]
     {
       V m[10], K[NK];
@@ -606,16 +620,69 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
         V ap, am;
         if (c < 2) push3<3, V, T>(Xg[3 * c][p], Xg[3 * c + 1][p], Xg[3 * c + 2][p], ap, am, A0[3 * c + p]);
         else push3<2, V, T>(Xg[6][p], Xg[7][p], Xg[7][p], ap, am, A0[6 + p]);
-        sts_pair_if(st_ap, s_ap + (3 * c + p) * YPF + oAP, ap);
-        sts_pair_if(st_am, s_am + (3 * c + p) * YPF + oAM, am);
+        sts_pair_if(st_ap, s_ap + (3 * c + p) * YPF + oAP + yoff, ap);
+        sts_pair_if(st_am, s_am + (3 * c + p) * YPF + oAM + yoff, am);
       }
   };
   // the y-push terms of a plane are complete: a barrier among the flow warps and the halo-row warp only
   auto xpass_barrier = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(C::NXPASS) : "memory"); };
 
-  if (flow || halow) {
+  // C: finish the y-pass of a source plane (a+ from the row below, a- from the row above, the rows' own a0)
+  // and z-push: am completes the plane below the source plane (-> outm), a0 / ap go on into the accumulators
+  auto cstage = [&](const T *yu, const T *yd, auto a0at, V (&accA)[10], V (&accB)[10], V (&outm)[10]) {
+    // moment index of (p,q,rr)
+    constexpr int MI[3][3][3] = {{{0, 3, 6}, {2, 9, -1}, {5, -1, -1}}, {{1, 8, -1}, {7, -1, -1}, {-1, -1, -1}}, {{4, -1, -1}, {-1, -1, -1}, {-1, -1, -1}}};
+#pragma unroll
+    for (int p = 0; p < 3; ++p) {
+      V Yq[3][3];   // [q][c]
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        const V up = lds_pair(yu + (3 * c + p) * YPF);
+        const V dn = lds_pair(yd + (3 * c + p) * YPF);
+        pull3<V, T>(up, dn, a0at(3 * c + p), Yq[0][c], Yq[1][c], Yq[2][c]);
+      }
+#pragma unroll
+      for (int q = 0; q + p <= 2; ++q) {
+        V ap, am, a0;
+        push3<3, V, T>(Yq[q][0], Yq[q][1], Yq[q][2], ap, am, a0);   // ap -> plane k+1, am -> plane k-1
+        {
+          const int m = MI[p][q][0];
+          outm[m] = accA[m] + am; accA[m] = accB[m] + a0; accB[m] = ap;
+        }
+        if (p + q <= 1) {
+          const int m = MI[p][q][1];
+          outm[m] = accA[m] - am; accA[m] = accB[m]; accB[m] = ap;
+        }
+        if (p + q == 0) {
+          const int m = MI[p][q][2];
+          outm[m] = pfma(am, T(2.0 / 3.0), accA[m]);
+          accA[m] = pfma(a0, T(-1.0 / 3.0), accB[m]);
+          accB[m] = ap * T(2.0 / 3.0);
+        }
+      }
+    }
+  };
+
+  if (UNI && (flow || halow)) {
+    // ============================ UNI: A warps (x-pass and y-push terms of the eight region rows) ============================
+    bool odd = kst & 1;                      // parity of plane k: the copy of the y-push fields it goes to
+    for (int i = 0; i < NI; ++i) {
+      asm volatile("" : "+r"(oM), "+r"(oT), "+r"(oAP), "+r"(oXP), "+r"(oXM), "+r"(oPL), "+r"(oPR));
+      if (i <= IZ1) mbar_wait(&bars[s], mph);
+      if (i >= I0 - 1 && i <= IZ1) {         // plane k is a source plane of this chunk
+        V A0[9];
+        xpass(odd, s, A0);
+        if (flow) {                          // the tile rows' own terms -> the C warps
+          T *a0 = s_a0 + (odd ? C::NYP * TLE : 0) + oT;
+#pragma unroll
+          for (int q = 0; q < 9; ++q) sts_pair(a0 + q * TLE, A0[q]);
+        }
+      }
+      odd = !odd;
+      iter_end(IC<0>(), i);
+    }
+  } else if (flow || halow) {
     // ============================ flow warps and the halo-row warp ============================
-    if (UNI) asm volatile("setmaxnreg.inc.sync.aligned.u32 248;");
     V accA[10], accB[10];     // Hermite moments being accumulated for planes k and k+1
     V ubx(T(0)), uby(T(0)), ubz(T(0)), rinv(T(1));   // u_b and 1/rho' of the plane completed last
 #pragma unroll
@@ -642,8 +709,8 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
       if (src) xpass(odd, s, A0);
       xpass_barrier();
       if (TWO && !UNI && halow && i <= IZ1 && i >= I0 + 1) {
-        phase_D(IC<0>(), dZ, dT, s, BUF - bo, deoff, demask, design);
-        phase_D(IC<4>(), dZ, dT, s, BUF - bo, deoff, demask, design);
+        phase_D(IC<0>(), dZ, dT, s, BUF - bo, deoff, demask, design, nullptr);
+        phase_D(IC<4>(), dZ, dT, s, BUF - bo, deoff, demask, design, nullptr);
       }
       V o[NF_MAX];
       if (TWO && flow && (unsigned)(i + ju) < (unsigned)njs) {
@@ -655,40 +722,9 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
         store_pair<T, FM_U, SLAB>(P, o, pst, kst + i - 2, gx_, gy_, img0, fs);
       }
       if (flow && src) {
-        // C: finish the y-pass of plane k (a+ from the row below, a- from the row above, own a0) and z-push
-        const T *yu = s_ap + oT, *yd = s_am + oT;
+        // C of plane k: plane k-1 is complete
         V outm[10];
-        // moment index of (p,q,rr)
-        constexpr int MI[3][3][3] = {{{0, 3, 6}, {2, 9, -1}, {5, -1, -1}}, {{1, 8, -1}, {7, -1, -1}, {-1, -1, -1}}, {{4, -1, -1}, {-1, -1, -1}, {-1, -1, -1}}};
-#pragma unroll
-        for (int p = 0; p < 3; ++p) {
-          V Yq[3][3];   // [q][c]
-#pragma unroll
-          for (int c = 0; c < 3; ++c) {
-            const V up = lds_pair(yu + (3 * c + p) * YPF);
-            const V dn = lds_pair(yd + (3 * c + p) * YPF);
-            pull3<V, T>(up, dn, A0[3 * c + p], Yq[0][c], Yq[1][c], Yq[2][c]);
-          }
-#pragma unroll
-          for (int q = 0; q + p <= 2; ++q) {
-            V ap, am, a0;
-            push3<3, V, T>(Yq[q][0], Yq[q][1], Yq[q][2], ap, am, a0);   // ap -> plane k+1, am -> plane k-1
-            {
-              const int m = MI[p][q][0];
-              outm[m] = accA[m] + am; accA[m] = accB[m] + a0; accB[m] = ap;
-            }
-            if (p + q <= 1) {
-              const int m = MI[p][q][1];
-              outm[m] = accA[m] - am; accA[m] = accB[m]; accB[m] = ap;
-            }
-            if (p + q == 0) {
-              const int m = MI[p][q][2];
-              outm[m] = pfma(am, T(2.0 / 3.0), accA[m]);
-              accA[m] = pfma(a0, T(-1.0 / 3.0), accB[m]);
-              accB[m] = ap * T(2.0 / 3.0);
-            }
-          }
-        }
+        cstage(s_ap + oT, s_am + oT, [&](int q) { return A0[q]; }, accA, accB, outm);
         // a4: plane k-1 is complete: u_b = m'/rho', Pi^neq' = Pi' - rho' u_b u_b (Hermite form)
         rinv = prcp<T>(outm[0] + V(T(1)));
         ubx = outm[1] * rinv; uby = outm[2] * rinv; ubz = outm[3] * rinv;
@@ -712,23 +748,58 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
       odd = !odd;
       iter_end(IC<0>(), i);
     }
-  } else if (colw || dwarp) {
-    // ============================ halo-column warp ============================
-    if (UNI) asm volatile("setmaxnreg.dec.sync.aligned.u32 112;");
-    if (dwarp) {
-      // UNI: the other three warps of its warpgroup run D (it carries no state from plane to plane)
+  } else if (colw || cwarp) {
+    if (UNI) asm volatile("setmaxnreg.inc.sync.aligned.u32 200;");
+    if (cwarp) {
+      // ============================ UNI: C warps ============================
+      // iteration k: C of source plane k-1 (terms the A warps left in iteration k-1): plane k-2 is complete
+      // and, with the F(k-2) formed in iteration k-1, finished and stored; then D: kappa, F of plane k-1
+      V accA[10], accB[10], Fr[3];
+#pragma unroll
+      for (int m = 0; m < 10; ++m) { accA[m] = V(T(0)); accB[m] = V(T(0)); }
+      Fr[0] = Fr[1] = Fr[2] = V(T(0));
+      const int jlo = max(z0, P.jet_lo ? 1 : 0);
+      const int njs = (gx_ >= xs && gy_ >= ys) ? min(z1, P.out_hi ? L.nz - 1 : L.nz) - jlo : 0;
+      T *pst = P.out.f[0] + o00 + (long long)(kst - 2) * L.plane;   // field 0 of the pair, plane k-2
+      const int ju = kst - 2 - jlo;            // (plane k-2) - jlo = i + ju
       const int oZ = r * ZW + 2 + 2 * lx;
       const int eoff = (lx == 0 ? C::B_ZL : (lx == LX - 1 ? C::B_ZL + RY : C::B_ZZ)) + 2 + r;
       const V emask(lx == 0 ? T(1) : T(0), lx == LX - 1 ? T(1) : T(0));
       const T esign = lx == 0 ? T(-0.5) : T(0.5);
-      int bo = (kst & 1) * BUF;
+      bool odd = kst & 1;                      // parity of plane k
       for (int i = 0; i < NI; ++i) {
-        const int bn = BUF - bo;
-        if (i <= IZ1 && i >= I0 + 1) phase_D(IC<0>(), oZ, oT, s, bn, eoff, emask, esign);
-        bo = bn;
+        asm volatile("" : "+r"(oT));
+        const int bn = odd ? 0 : BUF;          // half of the exchange block of plane k-1
+        if (i >= I0 && i <= IZ1 + 1) {
+          const int cp = odd ? 0 : C::NYP;     // fields of the copy of plane k-1
+          const T *a0 = s_a0 + cp * TLE + oT;
+          V outm[10];
+          cstage(s_ap + cp * YPF + oT, s_am + cp * YPF + oT, [&](int q) { return lds_pair(a0 + q * TLE); }, accA, accB, outm);
+          // a4, a6, a9: u_b = m'/rho', u' = u_b + F/rho', Pi^neq' = Pi' - rho' u_b u_b (Hermite form)
+          if ((unsigned)(i + ju) < (unsigned)njs) {
+            const V rinv = prcp<T>(outm[0] + V(T(1)));
+            const V ubx = outm[1] * rinv, uby = outm[2] * rinv, ubz = outm[3] * rinv;
+            V o[NF_MAX];
+            o[0] = outm[0];
+            o[1] = pfma(Fr[0], rinv, ubx);
+            o[2] = pfma(Fr[1], rinv, uby);
+            o[3] = pfma(Fr[2], rinv, ubz);
+            o[4] = outm[4] - outm[1] * ubx;
+            o[5] = outm[5] - outm[2] * uby;
+            o[6] = outm[6] - outm[3] * ubz;
+            o[7] = outm[7] - outm[1] * uby;
+            o[8] = outm[8] - outm[1] * ubz;
+            o[9] = outm[9] - outm[2] * ubz;
+            store_pair<T, FM_FLOW, SLAB>(P, o, pst, kst + i - 2, gx_, gy_, img0, fs);
+          }
+        }
+        if (i <= IZ1 && i >= I0 + 1) phase_D(IC<0>(), oZ, oT, s, bn, eoff, emask, esign, Fr);
+        pst += L.plane;
+        odd = !odd;
         iter_end(IC<0>(), i);
       }
     } else {
+    // ============================ halo-column warp ============================
     // node pairs: lanes 0 .. 2 RY - 1 own the two halo columns; every lane owns a pair of the halo rows
     PhaseState<T> pc, ph_;
     pc.clear(); ph_.clear();
@@ -799,7 +870,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
         mbar_wait(&bars[s], mph);
         if (UNI) {
           // one pair per thread; the warp of the halo rows runs the same code and stores nothing
-          // (D: the three spare warps of the halo-column warp's warpgroup)
+          // (D: the C warps)
           const V f0 = phase_B(IC<0>(), IC<0>(), p0, g0, s, bo, bn);
           const bool in0 = (unsigned)(i + pju) < (unsigned)pnjs0;
           stg_pair_if(in0, pph, f0);
@@ -808,7 +879,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
             o[F_PHI] = f0; store_rare<T, FM_PHI, SLAB>(P, o, kst + i - 1, gx_, gy_, img0);
           }
         } else {
-        if (i >= I0 + 1) phase_D(IC<0>(), g0.oZ, g0.oT, s, bn, eoff, emask, esign);   // (rows r + 2: the halo-row warp)
+        if (i >= I0 + 1) phase_D(IC<0>(), g0.oZ, g0.oT, s, bn, eoff, emask, esign, nullptr);   // (rows r + 2: the halo-row warp)
         const V f0 = phase_B(IC<0>(), IC<0>(), p0, g0, s, bo, bn);
         const V f1 = phase_B(IC<0>(), IC<2>(), p1, g0, s, bo, bn);
         // a9: phi'(k-1) of the two pairs
