@@ -327,11 +327,20 @@ def test_tile_multiple_grids_with_ragged_z(kernel, shape):
 
 @pytest.mark.parametrize("shape", [(48, 12, 10), (100, 20, 6), (36, 9, 5), (72, 30, 19)])
 def test_ragged_tiles_tiled_kernel(shape):
-    """nx, ny not multiples of the 32x8 tile: the last tile is shifted back inside the grid."""
+    """nx, ny not multiples of the 32x8 tile (two-component fp64: 32x6): the last tile is shifted back inside the grid."""
     nx, ny, nz = shape
     prm = dict(nx=nx, ny=ny, nz=nz, omega=1.8, two_component=True, sigma=0.01, interface_width=3.0)
     check("rt%s" % (shape,), lambda: inputs.smooth_random(nx, ny, nz, seed=7), prm, 20, tslb.F64, tslb.KERNEL_TILED)
     check("rt%s" % (shape,), lambda: inputs.smooth_random(nx, ny, nz, seed=7), prm, 10, tslb.F32, tslb.KERNEL_TILED)
+
+
+@pytest.mark.parametrize("shape", [(32, 6, 4), (64, 7, 9), (34, 14, 3), (96, 13, 70)])
+def test_fp64_two_component_tile_32x6(shape):
+    """The two-component fp64 build marches 32x6 tiles: the smallest grids it takes, a tile column
+    that is shifted back by all but one row, and a z extent of more than one 64-plane chunk."""
+    nx, ny, nz = shape
+    prm = dict(nx=nx, ny=ny, nz=nz, omega=1.8, two_component=True, sigma=0.01, interface_width=3.0)
+    check("u6%s" % (shape,), lambda: inputs.smooth_random(nx, ny, nz, seed=17), prm, 20, tslb.F64, tslb.KERNEL_TILED)
 
 
 def test_production_shape_slab_400x400():
