@@ -157,6 +157,7 @@ struct TiledMaps {
   CUtensorMap mom;   // 4-D (px, py, nz, 10) over the SOURCE buffer, box (RX, RY, 1, 10)
   CUtensorMap phi;   // 3-D (px, py, nz) over the source phi, box (RX, RYP, 1)
   int ntx, nty;      // tiles per row / column
+  unsigned fsh;      // half the spacing of the field arrays of a buffer, in bytes
   int zc;            // planes per z chunk
 };
 
@@ -300,15 +301,15 @@ __device__ __forceinline__ void store_rare(const StepParams<T> &P, const Pair<T>
   }
 }
 // Store the fields of MASK (bit m = field m) of one node pair of plane j.  p0: field 0 at this pair and
-// plane; the field arrays of a buffer are equally spaced (fs elements).
+// plane; the field arrays of a buffer are equally spaced (fsh = half the spacing in bytes, 32 bits: the address
+// of field m is then ONE multiply-add, IMAD.WIDE.U32).
 template <typename T, unsigned MASK, bool SLAB>
 __device__ __forceinline__ void store_pair(const StepParams<T> &P, const Pair<T> *o, T *p0, int j, int gx, int gy, bool img,
-                                           long long fs) {
-  T *p = p0;
-  int last = 0;
+                                           unsigned fsh) {
 #pragma unroll
   for (int m = 0; m < NF_MAX; ++m)
-    if (MASK >> m & 1u) { p += (m - last) * fs; last = m; *reinterpret_cast<Pair<T> *>(p) = o[m]; }
+    if (MASK >> m & 1u)
+      *reinterpret_cast<Pair<T> *>(reinterpret_cast<char *>(p0) + (unsigned long long)fsh * (unsigned)(2 * m)) = o[m];
   store_rare<T, MASK, SLAB>(P, o, j, gx, gy, img);
 }
 // predicated global pair store (one instruction, no branch)
@@ -424,7 +425,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
 
   const V omc(P.omc);
   const T w1 = T(1.0 / 6.0), w0 = T(2.0 / 3.0);
-  const long long fs = P.out.f[1] - P.out.f[0];          // field arrays are equally spaced
+  const unsigned fs = M.fsh;                             // field arrays are equally spaced: half the spacing in bytes
 
   // global coordinates / store offset (plane 0) of the thread's (first) pair
   const int gx_ = x0 + 2 * lx, gy_ = y0 + r - 1;
@@ -949,6 +950,8 @@ inline bool tiled_plan_create(TiledPlan &pl, int precision, const Layout &L, voi
   const int RX = pl.tx + 2 * (es == 4 ? 4 : 2), RY = pl.ty + 2, RYP = pl.ty + 4;
   for (int b = 0; b < 2; ++b) {
     const size_t fstride = (size_t)((char *)fields[b][1] - (char *)fields[b][0]);
+    if (fstride % 2 || fstride / 2 > 0xffffffffull) { why = "field arrays more than 8 GB apart"; return false; }
+    pl.maps[b].fsh = (unsigned)(fstride / 2);
     cuuint64_t gdim[4] = {(cuuint64_t)L.px, (cuuint64_t)L.py, (cuuint64_t)(L.nz + 2 * L.gz), 10};
     const size_t zoff = (size_t)L.gz * (size_t)L.plane * es;     // fields[][] point at plane 0
     cuuint64_t gstr[3] = {(cuuint64_t)L.px * es, (cuuint64_t)L.plane * es, (cuuint64_t)fstride};
