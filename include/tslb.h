@@ -51,8 +51,9 @@ enum { TSLB_BC_PERIODIC = 0, TSLB_BC_JET_INFLOW = 1, TSLB_BC_OUTFLOW = 2, TSLB_B
 enum {
   TSLB_KERNEL_AUTO = 0,     /* fastest kernel that supports the grid                           */
   TSLB_KERNEL_GENERIC = 1,  /* one thread per node, direct global loads; any grid size         */
-  TSLB_KERNEL_TILED = 2     /* TMA-staged 32x8 x-y tiles marching along z; needs nx >= 32, ny >= 8
-                               and nx a multiple of 4 (fp32) / 2 (fp64); a ragged last tile is
+  TSLB_KERNEL_TILED = 2     /* TMA-staged 32x8 x-y tiles (two-component fp64: 32x6) marching along z;
+                               needs nx >= 32, ny >= 8 (two-component fp64: 6) and nx a multiple of 4
+                               (fp32) / 2 (fp64), field arrays at most 8 GB apart; a ragged last tile is
                                shifted back inside the grid (tslb_create fails with TSLB_EINVAL
                                when the grid is not supported)                                 */
 };

@@ -105,7 +105,7 @@ Validated validate(const tslb_params *p) {
   v.L = make_layout(p->nx, p->ny, p->nz, v.slab ? GZ : 0);
   const bool tiled_ok = tiled_supported(p->precision, p->two_component != 0, p->nx, p->ny, p->nz);
   if (p->kernel == TSLB_KERNEL_TILED && !tiled_ok)
-    return fail("TSLB_KERNEL_TILED needs nx >= 32, ny >= 8 and nx a multiple of 4 (fp32) or 2 (fp64)");
+    return fail("TSLB_KERNEL_TILED needs nx >= 32, ny >= 8 (two-component fp64: 6) and nx a multiple of 4 (fp32) or 2 (fp64)");
   v.kernel = (p->kernel == TSLB_KERNEL_GENERIC || !tiled_ok || guo) ? TSLB_KERNEL_GENERIC : TSLB_KERNEL_TILED;
   // 2 buffers x nfields arrays, + 3 scratch arrays (n) for the generic two-component path,
   // + 3 more (F) for TSLB_FORCING_GUO
