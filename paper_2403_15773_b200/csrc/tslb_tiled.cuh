@@ -300,6 +300,14 @@ __device__ __forceinline__ void store_rare(const StepParams<T> &P, const Pair<T>
     }
   }
 }
+// streaming global pair store (st.global.cs: the new moments are not read again in this step, and should not push the
+// old moments that a neighbouring tile is about to read out of L2)
+__device__ __forceinline__ void stg_stream(float *a, Pair<float> v) {
+  asm volatile("st.global.cs.v2.f32 [%0], {%1, %2};" ::"l"(a), "f"(v.x), "f"(v.y) : "memory");
+}
+__device__ __forceinline__ void stg_stream(double *a, Pair<double> v) {
+  asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};" ::"l"(a), "d"(v.x), "d"(v.y) : "memory");
+}
 // Store the fields of MASK (bit m = field m) of one node pair of plane j.  p0: field 0 at this pair and
 // plane; the field arrays of a buffer are equally spaced (fsh = half the spacing in bytes, 32 bits: the address
 // of field m is then ONE multiply-add, IMAD.WIDE.U32).
@@ -309,16 +317,16 @@ __device__ __forceinline__ void store_pair(const StepParams<T> &P, const Pair<T>
 #pragma unroll
   for (int m = 0; m < NF_MAX; ++m)
     if (MASK >> m & 1u)
-      *reinterpret_cast<Pair<T> *>(reinterpret_cast<char *>(p0) + (unsigned long long)fsh * (unsigned)(2 * m)) = o[m];
+      stg_stream(reinterpret_cast<T *>(reinterpret_cast<char *>(p0) + (unsigned long long)fsh * (unsigned)(2 * m)), o[m]);
   store_rare<T, MASK, SLAB>(P, o, j, gx, gy, img);
 }
 // predicated global pair store (one instruction, no branch)
 __device__ __forceinline__ void stg_pair_if(bool p, float *a, Pair<float> v) {
-  asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %0, 0;\n@q st.global.v2.f32 [%1], {%2, %3};\n}"
+  asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %0, 0;\n@q st.global.cs.v2.f32 [%1], {%2, %3};\n}"
                ::"r"((int)p), "l"(a), "f"(v.x), "f"(v.y) : "memory");
 }
 __device__ __forceinline__ void stg_pair_if(bool p, double *a, Pair<double> v) {
-  asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %0, 0;\n@q st.global.v2.f64 [%1], {%2, %3};\n}"
+  asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %0, 0;\n@q st.global.cs.v2.f64 [%1], {%2, %3};\n}"
                ::"r"((int)p), "l"(a), "d"(v.x), "d"(v.y) : "memory");
 }
 constexpr unsigned FM_U = 0xEu, FM_RHOPI = 0x3F1u, FM_FLOW = 0x3FFu, FM_PHI = 0x400u;   // field masks
