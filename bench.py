@@ -464,7 +464,7 @@ def main():
     traffic = None
     tp = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tp):
-        tj = json.load(open(tp)).get(args.config)
+        tj = json.load(open(tp)).get(args.config + ("" if args.precision == "f32" else "_" + args.precision))
         if tj and kname.startswith("tiled<"):     # the ncu capture is of the tiled kernel
             traffic = tj.get("dram_bytes_per_launch")
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
