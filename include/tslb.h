@@ -235,6 +235,12 @@ long long tslb_launch_count(const tslb_ctx *c);
  * y in [0,ny) into out[nx*ny] doubles (host pointer) -- test probe for the bit-exact hash pin.  */
 int tslb_debug_xi(tslb_ctx *c, long long step, double *out_host);
 
+/* Test probe for the arithmetic of 1/rho' and |grad(phi)| in the tiled kernel ("fp32 / fp64
+ * arithmetic of 1/rho' and n"): evaluates, ON THE DEVICE and in the context's precision, the kernel's reciprocal and
+ * square root of in[0..n) (host doubles, converted to the context's precision) into out_rcp[n] and out_sqrt[n] (host
+ * doubles).  Synchronous; allocates and frees its own scratch.  TSLB_EINVAL for a NULL argument or n < 1.             */
+int tslb_debug_math(tslb_ctx *c, int n, const double *in_host, double *out_rcp_host, double *out_sqrt_host);
+
 /* Synchronise the stream, close imported neighbour handles, free what the library allocated (not a
  * caller-owned workspace).  NULL is accepted.  Always TSLB_OK.                                      */
 int tslb_destroy(tslb_ctx *c);

@@ -533,6 +533,16 @@ int physvel_noalloc_typed(tslb_ctx *c, void *const dst[3], void *scratch) {
 
 }  // namespace
 
+// probe of the tiled kernel's reciprocal and square root (tslb_debug_math)
+template <typename T>
+__global__ void debug_math_kernel(int n, const double *in, double *orcp, double *osqrt) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const T v = (T)in[i];
+  orcp[i] = (double)tslb::rcp1(v);
+  osqrt[i] = (double)tslb::sqrt1(v);
+}
+
 extern "C" {
 
 size_t tslb_workspace_bytes(const tslb_params *p) {
@@ -829,6 +839,25 @@ int tslb_debug_xi(tslb_ctx *c, long long step, double *out_host) {
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
   cudaFree(d);
   if (e != cudaSuccess) return c->cuda_fail(e, "tslb_debug_xi");
+  return TSLB_OK;
+}
+
+int tslb_debug_math(tslb_ctx *c, int n, const double *in_host, double *out_rcp_host, double *out_sqrt_host) {
+  if (!c || !in_host || !out_rcp_host || !out_sqrt_host || n < 1) return TSLB_EINVAL;
+  CK(cudaSetDevice(c->p.device));
+  double *d = nullptr;
+  CK(cudaMalloc(&d, sizeof(double) * 3 * (size_t)n));
+  cudaError_t e = cudaMemcpyAsync(d, in_host, sizeof(double) * n, cudaMemcpyHostToDevice, c->stream);
+  if (e == cudaSuccess) {
+    if (c->p.precision == TSLB_F32) debug_math_kernel<float><<<(n + 127) / 128, 128, 0, c->stream>>>(n, d, d + n, d + 2 * (size_t)n);
+    else debug_math_kernel<double><<<(n + 127) / 128, 128, 0, c->stream>>>(n, d, d + n, d + 2 * (size_t)n);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaMemcpyAsync(out_rcp_host, d + n, sizeof(double) * n, cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(out_sqrt_host, d + 2 * (size_t)n, sizeof(double) * n, cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  cudaFree(d);
+  if (e != cudaSuccess) return c->cuda_fail(e, "tslb_debug_math");
   return TSLB_OK;
 }
 

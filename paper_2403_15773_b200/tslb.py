@@ -21,7 +21,7 @@ FORCING_KICK, FORCING_GUO = 0, 1
 EXPORTS = ["tslb_workspace_bytes", "tslb_create", "tslb_init_fields", "tslb_step",
            "tslb_get_moments", "tslb_get_physical_velocity", "tslb_get_physical_velocity_noalloc",
            "tslb_noalloc_scratch_bytes", "tslb_step_count", "tslb_kernel_name", "tslb_launch_count",
-           "tslb_debug_xi", "tslb_destroy", "tslb_last_error", "tslb_workspace_ptr",
+           "tslb_debug_xi", "tslb_debug_math", "tslb_destroy", "tslb_last_error", "tslb_workspace_ptr",
            "tslb_attach_neighbor", "tslb_ipc_get_handle", "tslb_attach_neighbor_ipc", "tslb_detach_neighbors", "tslb_halo_push",
            "tslb_stats_begin", "tslb_stats_get", "tslb_stats_end"]
 
@@ -80,6 +80,7 @@ def lib():
         L.tslb_launch_count.argtypes = [vp]
         L.tslb_launch_count.restype = ctypes.c_longlong
         L.tslb_debug_xi.argtypes = [vp, ctypes.c_longlong, ctypes.POINTER(ctypes.c_double)]
+        L.tslb_debug_math.argtypes = [vp, ctypes.c_int] + [ctypes.POINTER(ctypes.c_double)] * 3
         L.tslb_destroy.argtypes = [vp]
         L.tslb_last_error.argtypes = [vp]
         L.tslb_last_error.restype = ctypes.c_char_p
@@ -303,6 +304,16 @@ class Tslb:
     @property
     def launch_count(self):
         return lib().tslb_launch_count(self._h)
+
+    def debug_math(self, values):
+        """The tiled kernel's reciprocal and square root of `values`, evaluated on the device in the context's
+        precision (test probe)."""
+        v = np.ascontiguousarray(values, dtype=np.float64).ravel()
+        pd = ctypes.POINTER(ctypes.c_double)
+        rcp, sq = np.empty_like(v), np.empty_like(v)
+        self._check(lib().tslb_debug_math(self._h, int(v.size), v.ctypes.data_as(pd), rcp.ctypes.data_as(pd),
+                                          sq.ctypes.data_as(pd)))
+        return rcp, sq
 
     def debug_xi(self, step):
         nz, ny, nx = self.shape

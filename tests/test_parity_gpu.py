@@ -303,6 +303,35 @@ def test_p13_inflow_hash_bit_exact(precision):
         assert np.array_equal(dev, exp)
 
 
+@pytest.mark.parametrize("precision", [tslb.F64, tslb.F32])
+def test_kernel_reciprocal_and_root_against_ieee(precision):
+    """the tiled kernel's own 1/x and sqrt(x) (MUFU seed + Newton steps in fp64, the MUFU
+    approximations in fp32) against the IEEE results numpy gives: within 1 ulp (fp64) / 2 ulp (fp32) over the ranges the
+    step uses them on (rho' ~ 1, |G| + 1e-12, G.G), sqrt(0) = 0, and in fp64 a root below 1e-140 returned as 0."""
+    rng = np.random.default_rng(5)
+    v = np.concatenate([10.0 ** rng.uniform(-12, 1, 4000), rng.uniform(0.5, 2.0, 4000), 10.0 ** rng.uniform(-24, -12, 2000),
+                        [1.0, 0.25, 1e-12, 2.0 / 3.0, 1.0 + 2.0 ** -52]])
+    g = tslb.Tslb(32, 8, 4, 1.5, precision=precision, two_component=True, sigma=0.01, interface_width=3.0)
+    try:
+        dt = np.float64 if precision == tslb.F64 else np.float32
+        vv = v.astype(dt)
+        rcp, sq = g.debug_math(vv)
+        ulps = 1.0 if precision == tslb.F64 else 2.0
+        er = np.abs(rcp.astype(dt) - (dt(1) / vv)) / np.spacing(dt(1) / vv)
+        es = np.abs(sq.astype(dt) - np.sqrt(vv)) / np.spacing(np.sqrt(vv))
+        print("rcp ulp max", er.max(), "sqrt ulp max", es.max())
+        assert er.max() <= ulps and es.max() <= ulps
+        tiny = np.array([0.0, 5e-324, 1e-310, 1e-300, 9e-281]) if precision == tslb.F64 else np.array([0.0])
+        _, sq0 = g.debug_math(tiny)
+        assert np.array_equal(sq0, np.zeros_like(sq0))
+        if precision == tslb.F64:
+            big = 10.0 ** rng.uniform(-279, -24, 2000)
+            _, sqb = g.debug_math(big)
+            assert (np.abs(sqb - np.sqrt(big)) <= np.spacing(np.sqrt(big))).all()
+    finally:
+        g.close()
+
+
 # ------------------------------------------------------------------ edge cases
 @pytest.mark.parametrize("precision", [tslb.F64, tslb.F32])
 @pytest.mark.parametrize("shape", [(20, 12, 10), (33, 17, 9), (3, 3, 3), (1, 1, 1), (64, 8, 5)])
