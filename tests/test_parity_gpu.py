@@ -450,20 +450,21 @@ def test_device_pointers_and_torch_stream():
     assert np.array_equal(md["pineq"].cpu().numpy(), mh["pineq"])
 
 
+@pytest.mark.parametrize("precision", [tslb.F32, tslb.F64])
 @pytest.mark.parametrize("kernel", KERNELS)
 @pytest.mark.parametrize("jet", [False, True])
-def test_step_n_as_a_replayed_graph_equals_single_steps(kernel, jet):
+def test_step_n_as_a_replayed_graph_equals_single_steps(kernel, jet, precision):
     """tslb_step(n >= 5) replays a captured CUDA graph of two steps (the inflow hash then reads its step index
     from a device counter); it must give the bits of n calls of tslb_step(1), from either starting buffer."""
     if jet:
         prm = inputs.jet_params(64, 32, 24, D=9, U=0.04, Re=300.0, We=50.0, perturbation=0.1, seed=5)
-        d = round_inputs(inputs.jet_developed(64, 32, 24, D=9, ndrop=5), tslb.F32)
+        d = round_inputs(inputs.jet_developed(64, 32, 24, D=9, ndrop=5), precision)
     else:
         prm = dict(nx=64, ny=32, nz=24, omega=1.8, two_component=True, sigma=0.01, interface_width=3.0)
-        d = round_inputs(inputs.smooth_random(64, 32, 24, seed=2), tslb.F32)
+        d = round_inputs(inputs.smooth_random(64, 32, 24, seed=2), precision)
     res = []
     for mode in ("graph", "single"):
-        g = tslb.Tslb(prm["nx"], prm["ny"], prm["nz"], prm["omega"], precision=tslb.F32, kernel=kernel, **gpu_kwargs(prm))
+        g = tslb.Tslb(prm["nx"], prm["ny"], prm["nz"], prm["omega"], precision=precision, kernel=kernel, **gpu_kwargs(prm))
         g.init_fields(d["rho"], d["ux"], d["uy"], d["uz"], d.get("phi"), d.get("pineq"))
         for n in (13, 1, 8):                       # odd first call: the second graph starts from the other buffer
             if mode == "graph":
