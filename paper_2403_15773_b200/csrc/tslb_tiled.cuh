@@ -713,6 +713,16 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
       asm volatile("" : "+r"(oM), "+r"(oT), "+r"(oAP), "+r"(oXP), "+r"(oXM), "+r"(oPL), "+r"(oPR));
       const int bo = odd ? BUF : 0;
       if (i >= (TWO ? 0 : 1) && i <= IZ1) mbar_wait(&bars[s], mph);
+      if (TWO && flow && (unsigned)(i + ju) < (unsigned)njs) {
+        // a6: u'(k-2) = u_b + F / rho' with the F(k-2) the phase warps wrote in iteration k-1; a9: store it.
+        // (First thing in the iteration: u_b and 1/rho' die before the x-pass, and the loads overlap its own.)
+        V o[NF_MAX];
+        const T *kf = s_buf + bo + C::B_KF + oT;
+        o[1] = pfma(lds_pair(kf), rinv, ubx);
+        o[2] = pfma(lds_pair(kf + TLE), rinv, uby);
+        o[3] = pfma(lds_pair(kf + 2 * TLE), rinv, ubz);
+        store_pair<T, FM_U, SLAB>(P, o, pst, kst + i - 2, gx_, gy_, img0, fs);
+      }
       const bool src = i >= I0 - 1 && i <= IZ1;    // plane k is a source plane of this chunk
       V A0[9];                               // own y-push term a0 per (c,p)
       if (src) xpass(odd, s, A0);
@@ -722,14 +732,6 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
         phase_D(IC<4>(), dZ, dT, s, BUF - bo, deoff, demask, design, nullptr);
       }
       V o[NF_MAX];
-      if (TWO && flow && (unsigned)(i + ju) < (unsigned)njs) {
-        // a6: u'(k-2) = u_b + F / rho' with the F(k-2) the phase warps wrote in iteration k-1; a9: store it
-        const T *kf = s_buf + bo + C::B_KF + oT;
-        o[1] = pfma(lds_pair(kf), rinv, ubx);
-        o[2] = pfma(lds_pair(kf + TLE), rinv, uby);
-        o[3] = pfma(lds_pair(kf + 2 * TLE), rinv, ubz);
-        store_pair<T, FM_U, SLAB>(P, o, pst, kst + i - 2, gx_, gy_, img0, fs);
-      }
       if (flow && src) {
         // C of plane k: plane k-1 is complete
         V outm[10];
