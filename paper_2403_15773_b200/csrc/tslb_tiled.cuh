@@ -198,6 +198,14 @@ __device__ __forceinline__ void sts_pair_if(bool p, double *a, Pair<double> v) {
                ::"r"((int)p), "r"(smem_u32(a)), "d"(v.x), "d"(v.y) : "memory");
 }
 
+// predicated shared-memory load into v (one predicated instruction, no branch)
+__device__ __forceinline__ void lds_if(int p, const float *a, float &v) {
+  asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %2, 0;\n@q ld.shared.f32 %0, [%1];\n}" : "+f"(v) : "r"(smem_u32(a)), "r"(p) : "memory");
+}
+__device__ __forceinline__ void lds_if(int p, const double *a, double &v) {
+  asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %2, 0;\n@q ld.shared.f64 %0, [%1];\n}" : "+d"(v) : "r"(smem_u32(a)), "r"(p) : "memory");
+}
+
 // The 1-D three-point operator of the tensor-product basis in PUSH form.  A source
 // node holding the un-normalised Hermite coefficients g_0, g_1, g_2 (index along this axis) sends
 //     a+ = g0/6 + g1/2 + g2/2   to the node at +1,
@@ -576,25 +584,21 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
   };
 
   // A: x-pass of region row r of plane k in push form, then the y-push terms (flow warps and the halo-row
-  // warp).  Each node's K is evaluated once; a+ / a- cross to the x-neighbour thread through shared memory
-  // (same warp); the lanes at the tile edge take the halo column's term, which the halo-column warp left in
-  // the extra row of the same fields one iteration earlier.
+  // warp).  Each node's K is evaluated once; a+ / a- cross to the x-neighbour thread by shuffle (through shared
+  // memory the store -> __syncwarp -> load chain sat on the critical path: +1.8 % in fp32); the lanes at the
+  // tile edge load the halo column's term instead, which the halo-column warp left in the extra row of the
+  // y-push fields one iteration earlier.
   const bool st_ap = r <= TY - 1, st_am = r >= 2;        // rows 0..TY-1 send an a+, rows 2..TY+1 an a-
   // y-push fields: a+ is stored at row index r, a- at r-2; a tile row r reads both at index r-1 (= oT)
   int oAP = r * TX + 2 * lx;
-  // x-exchange word of this lane: word `lane` of a row of the y-push fields 0..7 that this warp is about
-  // to overwrite (a+ field: the warp's first sending row; a- field: its last)
-  int oXP = (flow ? 2 * wid + 1 : 0) * TX + lane, oXM = (flow ? 2 * wid : TY - 1) * TX + lane;
-  // the word it reads: its x neighbour's, or (lanes at the tile edge) the halo-column term of row r in the
-  // extra row of the same field (+ RY for planes of odd parity)
-  int oPL = lx == 0 ? TY * TX + r : oXP - 1, oPR = lx == LX - 1 ? TY * TX + r : oXM + 1;
+  // the word a lane at the tile edge loads: the halo-column term of row r in the extra row of the y-push
+  // fields 0..7 of copy 0 (+ RY for planes of odd parity)
+  int oPL = TY * TX + r;
   const int hpar = (lx == 0 ? 1 : 0) | (lx == LX - 1 ? 2 : 0);
   auto xpass = [&](bool odd, int s, V (&A0)[9]) {      // odd: parity of the plane
     const int oAM = oAP - 2 * TX;
     const int yoff = UNI && odd ? C::NYP * YPF : 0;    // UNI: the copy of the y-push fields of this parity
-    T *const xp = s_ap + oXP + yoff, *const xm = s_am + oXM + yoff;
-    const int hoff = odd ? RY : 0;                     // (the halo-column terms: always in copy 0)
-    const T *pl = s_ap + oPL + ((hpar & 1) ? hoff : yoff), *pr = s_am + oPR + ((hpar & 2) ? hoff : yoff);
+    const T *pl = s_ap + oPL + (odd ? RY : 0), *pr = s_am + oPL + (odd ? RY : 0);
     V Xg[8][3];   // [group][p]
     {
       V m[10], K[NK];
@@ -611,15 +615,13 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
       push3<1, V, T>(K[K021], K[K021], K[K021], gp[5], gm[5], g0[5]);   // (2,1)
       push3<2, V, T>(K[K002], K[K102], K[K102], gp[6], gm[6], g0[6]);   // (0,2)
       push3<1, V, T>(K[K012], K[K012], K[K012], gp[7], gm[7], g0[7]);   // (1,2)
-      // lane l of the warp parks gp.y / gm.x at word l of one of the warp's own y-push rows
-#pragma unroll
-      for (int g = 0; g < 8; ++g) { xp[g * YPF] = gp[g].y; xm[g * YPF] = gm[g].x; }
-      __syncwarp();
 #pragma unroll
       for (int g = 0; g < 8; ++g) {
-        pull3s<V, T>(pl[g * YPF], gp[g].x, gm[g].y, pr[g * YPF], g0[g], Xg[g][0], Xg[g][1], Xg[g][2]);
+        T l = __shfl_up_sync(0xffffffffu, gp[g].y, 1, LX), q = __shfl_down_sync(0xffffffffu, gm[g].x, 1, LX);
+        lds_if(hpar & 1, pl + g * YPF, l);
+        lds_if(hpar & 2, pr + g * YPF, q);
+        pull3s<V, T>(l, gp[g].x, gm[g].y, q, g0[g], Xg[g][0], Xg[g][1], Xg[g][2]);
       }
-      __syncwarp();
     }
     // y-push per (c, p): groups of c = 0: b = 0,1,2 -> g 0,1,2; c = 1: g 3,4,5; c = 2: b = 0,1 -> g 6,7
 #pragma unroll
@@ -676,7 +678,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     // ============================ UNI: A warps (x-pass and y-push terms of the eight region rows) ============================
     bool odd = kst & 1;                      // parity of plane k: the copy of the y-push fields it goes to
     for (int i = 0; i < NI; ++i) {
-      asm volatile("" : "+r"(oM), "+r"(oT), "+r"(oAP), "+r"(oXP), "+r"(oXM), "+r"(oPL), "+r"(oPR));
+      asm volatile("" : "+r"(oM), "+r"(oT), "+r"(oAP), "+r"(oPL));
       if (i <= IZ1) mbar_wait(&bars[s], mph);
       if (i >= I0 - 1 && i <= IZ1) {         // plane k is a source plane of this chunk
         V A0[9];
@@ -710,7 +712,7 @@ tiled_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     const T design = lx == 0 ? T(-0.5) : T(0.5);
     for (int i = 0; i < NI; ++i) {
       // (keep the loop-invariant offsets in registers: recomputing them from the thread index costs more)
-      asm volatile("" : "+r"(oM), "+r"(oT), "+r"(oAP), "+r"(oXP), "+r"(oXM), "+r"(oPL), "+r"(oPR));
+      asm volatile("" : "+r"(oM), "+r"(oT), "+r"(oAP), "+r"(oPL));
       const int bo = odd ? BUF : 0;
       if (i >= (TWO ? 0 : 1) && i <= IZ1) mbar_wait(&bars[s], mph);
       if (TWO && flow && (unsigned)(i + ju) < (unsigned)njs) {
