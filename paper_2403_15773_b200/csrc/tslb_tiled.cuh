@@ -1031,18 +1031,19 @@ inline bool tiled_plan_create(TiledPlan &pl, int precision, const Layout &L, voi
     pl.maps[b].nty = (L.ny + pl.ty - 1) / pl.ty;
   }
   // z chunking: every chunk pays a 6-iteration pipeline prologue (three of them light), and the grid runs in
-  // waves of (CTAs per SM) x (SM count): pick the chunk length that minimises waves x (zc + 5) -- up to 64
-  // planes.  Longer chunks would save prologue iterations, but CTAs start in blockIdx order whenever a slot
-  // frees, so the y-neighbour of a tile (ntx launches later) runs behind it by a fixed fraction of a chunk: with
-  // 64 planes its halo rows are still in L2 when it reads them, with 256 they are not (C5: 22.2 GB of DRAM
-  // reads against 27.8 GB per step, 36.5 against 35.5 GLUPS; profiles/r02_zchunk_sweep.md).
+  // waves of (CTAs per SM) x (SM count): pick the chunk length that minimises waves x (zc + 5) -- up to 128
+  // planes.  Longer chunks save prologue iterations, but CTAs start in blockIdx order whenever a slot frees, so the
+  // y-neighbour of a tile (ntx launches later) runs behind it by a fixed fraction of a chunk, and with long chunks
+  // its halo rows have left L2 when it reads them (DRAM reads of a C5 step: 22.2 GB at 64 planes, 25.3 at 128, 27.8
+  // at 256; profiles/r02_zchunk_sweep.md).  With the final kernels 128 planes measure best on C5 (39.9 against
+  // 39.4 GLUPS at 64 and 39.9 at 256, 60 steps).
   const long long tiles = (long long)pl.maps[0].ntx * pl.maps[0].nty;
   int nsm = 148;
   cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, device);
   const long long slots = (long long)nsm * (precision == TSLB_F32 ? 2 : 1);
   int zc = L.nz;
   long long best = -1;
-  for (int cand = 8; cand <= (precision == TSLB_F32 ? 64 : 128); cand *= 2) {   // (fp64: 128 measures 1 % better than 64)
+  for (int cand = 8; cand <= 128; cand *= 2) {
     const int c = cand < L.nz ? cand : L.nz;
     const long long ctas = tiles * ((L.nz + c - 1) / c);
     const long long cost = ((ctas + slots - 1) / slots) * (c + 5);
